@@ -1,0 +1,167 @@
+/*
+ * zmc.h -- C ABI of zmc_scan: batched direct Monte-Carlo integration over a parameter grid.
+ *
+ * What it computes (ZMCintegral-v5, arXiv 1910.01965; citations are PAPER.md lines):
+ *   f(x) = \int dy g(y; x),  y in a box of R^N, x = (x_1..x_M)            (Eq. 1)
+ * independently at every point x of the Cartesian product of M value lists,
+ * by the direct (plain) Monte-Carlo method, one integration per grid point
+ * (PAPER.md:65), with the grid cut into batches and the result returned as the
+ * "multi-dimensional grid with each element being the integrated values".
+ * HToD / DToH / evaluation times are reported separately as in the paper's tables
+ * (PAPER.md:85, :132-140).  Readings of everything the paper leaves open (RNG = Philox4x32-10,
+ * stream layout, uniforms, grid order, standard error) are listed in DESIGN.md "Readings".
+ *
+ * Conventions
+ *   - All `const double*` inputs (bounds, lists, consts) are HOST memory, copied before the call
+ *     returns; the library keeps no pointer to them.
+ *   - out_mean / out_stderr: G' elements each (G' = count of the scanned flat range, default the
+ *     whole grid G = prod(lists[i].count)), element r = flat index first_index + r, flat order is
+ *     row-major with the LAST list fastest.  Element type and location are set by zmc_options
+ *     (default: double, DEVICE memory).  The caller owns them; they must stay valid until
+ *     `stream` has been synchronised.
+ *   - The call only enqueues work: kernels on `stream`, result copies (host output) on an
+ *     internal side stream that is joined back into `stream`.  Results are valid after
+ *     cudaStreamSynchronize(stream).  If `timing` is non-NULL the call synchronises before
+ *     returning and fills it.
+ *   - Argument errors are detected before anything is enqueued and leave the outputs untouched.
+ *     No exception crosses this boundary.  There is no CPU fallback: without a usable CUDA device
+ *     every compute call returns ZMC_ERR_CUDA.
+ *   - Every random word is keyed by (seed, GLOBAL flat grid index, word index), so results do
+ *     not depend on batching, sub-ranges or launch shape (bit-identical for a fixed schedule).
+ */
+#ifndef ZMC_H_
+#define ZMC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define ZMC_API __attribute__((visibility("default")))
+#else
+#define ZMC_API
+#endif
+
+#define ZMC_MAX_N 16        /* integration dimensions */
+#define ZMC_MAX_M 8         /* parameters */
+#define ZMC_MAX_CONSTS 8    /* family constants */
+
+typedef enum zmc_status {
+    ZMC_OK = 0,
+    ZMC_ERR_INVALID_ARG = 1,       /* NULL pointer; N or M out of range; count < 1; !(a_k < b_k); non-finite
+                                      bound/value; n_samples < 2 or > 2^32-1 or n_samples*N > 2^34; bad option */
+    ZMC_ERR_UNKNOWN_INTEGRAND = 2,
+    ZMC_ERR_SHAPE_MISMATCH = 3,    /* (N, M, n_consts) not accepted by that family */
+    ZMC_ERR_GRID_TOO_LARGE = 4,    /* prod(count) > 2^48, or one list longer than 2^31-1 */
+    ZMC_ERR_OUT_OF_MEMORY = 5,
+    ZMC_ERR_CUDA = 6               /* see zmc_last_cuda_error() */
+} zmc_status;
+
+/* Integrand families g(y; x), SURVEY.md 8(c) S7 / BASELINE.json configs.  y_k is 0-based. */
+enum {
+    ZMC_FAM_C1_COS_XY = 1,        /* cos(x1*y0)                                   N=1, M=1 */
+    ZMC_FAM_C2_SIN_XY2 = 2,       /* sin(x1*y0 + x2*y1)                           N=2, M=2 */
+    ZMC_FAM_C3_OSCILLATORY = 3,   /* cos(2 pi u + sum_k c_k y_k), c_k = x_{(k mod 3)+1}*(k+1); consts = {u}; N>=1, M=3 */
+    ZMC_FAM_C4_GAUSS_PEAK = 4,    /* exp(-a^2 sum_k (y_k-w_k)^2), a=x1, w=(x2,x2,x3,x3,x4,x4)   N=6, M=4 */
+    ZMC_FAM_C5_DAMPED_COS = 5,    /* exp(-x1 |y|^2) cos(x2 y0+x3 y1+x4 y2) (1+x5 y0 y1 y2)      N=3, M=5 */
+    ZMC_FAM_P6_SIN_SUM = 6,       /* sin(sum_k y_k + sum_l x_l): Eq. (2), :120 Eq. (4); any N, M */
+    ZMC_FAM_CONST_ONE = 100,      /* 1 (diagnostic) */
+    ZMC_FAM_PARAM_ECHO = 101,     /* x_{i+1}, consts = {i} (diagnostic) */
+    ZMC_FAM_LIN_Y = 102,          /* y_k, consts = {k} (diagnostic) */
+    ZMC_FAM_POLY = 103            /* prod_k y_k (diagnostic) */
+};
+
+enum { ZMC_PREC_F64 = 0, ZMC_PREC_F32E = 1 };             /* F32E: fp32 evaluate, fp64 accumulate */
+enum { ZMC_OUT_F64 = 0, ZMC_OUT_F32 = 1 };
+enum { ZMC_LOC_DEVICE = 0, ZMC_LOC_HOST = 1 };            /* HOST: pinned memory recommended */
+enum { ZMC_SCHED_AUTO = 0, ZMC_SCHED_THREAD = 1, ZMC_SCHED_WARP = 2, ZMC_SCHED_CTA = 3 };
+enum { ZMC_FAST_MATH_DEFAULT = -1, ZMC_FAST_MATH_OFF = 0, ZMC_FAST_MATH_ON = 1 };
+
+/* One parameter's value list.  Host memory. */
+typedef struct zmc_param_list {
+    const double* values;
+    int64_t count;
+} zmc_param_list;
+
+/* Options of zmc_scan_ex.  Zero-initialise, set struct_size = sizeof(zmc_options), override fields. */
+typedef struct zmc_options {
+    uint32_t struct_size;
+    int32_t precision;       /* ZMC_PREC_*: arithmetic of the integrand evaluation (sums are always fp64) */
+    int32_t out_dtype;       /* ZMC_OUT_*: element type of out_mean / out_stderr */
+    int32_t out_location;    /* ZMC_LOC_*: where out_mean / out_stderr live */
+    int32_t schedule;        /* ZMC_SCHED_*: lanes per grid point (1 / 32 / one CTA); AUTO picks by (count, n_samples) */
+    int32_t fast_math;       /* ZMC_FAST_MATH_*: F32E only -- MUFU sin/cos/ex2 (default ON); ignored for F64 */
+    uint64_t batch_points;   /* grid points per batch; 0 = one batch */
+    uint64_t first_index;    /* scan only flat indices [first_index, first_index+count) ... */
+    uint64_t count;          /* ... 0 = up to the end of the grid */
+    const double* consts;    /* family constants (host), n_consts of them */
+    int32_t n_consts;
+    int32_t reserved;
+} zmc_options;
+
+/* Where the time went (the paper's HToD / DToH / GPU evaluation split). */
+typedef struct zmc_timing {
+    double h2d_ms;           /* staging of bounds/lists (device time) */
+    double kernel_ms;        /* sum of the batch kernels' device time */
+    double d2h_ms;           /* sum of the result copies' device time (host output only) */
+    double exposed_d2h_ms;   /* max(0, wall - h2d - kernel): copy time NOT hidden behind compute */
+    double wall_ms;          /* first enqueue to last completion, device time on `stream` */
+    int64_t n_batches;
+    int64_t gpu_launches;    /* kernels of this library launched by the call */
+    uint64_t d2h_bytes;
+    uint64_t h2d_bytes;
+    int32_t schedule;        /* the schedule actually used */
+    int32_t reserved;
+} zmc_timing;
+
+typedef struct zmc_integrand_info {
+    int32_t id;
+    const char* name;
+    int32_t N_min, N_max;    /* accepted integration dimensions */
+    int32_t M_min, M_max;    /* accepted parameter counts */
+    int32_t n_consts;
+    int32_t has_closed_form;
+} zmc_integrand_info;
+
+/*
+ * zmc_scan -- mean and standard error of the plain Monte-Carlo estimate at every grid point
+ * (PAPER.md:55-65).  Defaults: fp64 path, double outputs in DEVICE memory, one batch, AUTO schedule.
+ *   integrand_id  ZMC_FAM_*                       N        box dimensions, 1..ZMC_MAX_N
+ *   bounds        2N doubles a_0,b_0,..           M        number of lists, 1..ZMC_MAX_M
+ *   lists         M value lists                   n_samples samples per grid point (>= 2)
+ *   seed          Philox key                      stream   cudaStream_t (as void*), may be 0
+ * mean = V * avg(g),  stderr = V * sqrt(s^2 / n) with the unbiased (n-1) sample variance,
+ * V = prod_k (b_k - a_k).
+ */
+ZMC_API zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                    uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream);
+
+/* Same, with options (may be NULL = defaults) and an optional timing report (may be NULL). */
+ZMC_API zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                       uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream,
+                       const zmc_options* opt, zmc_timing* timing);
+
+/* Pure host helpers (no GPU needed). */
+ZMC_API int zmc_integrand_count(void);
+ZMC_API zmc_status zmc_integrand_info_at(int index, zmc_integrand_info* info);   /* index in [0, count) */
+ZMC_API zmc_status zmc_integrand_info_by_id(int integrand_id, zmc_integrand_info* info);
+ZMC_API const char* zmc_status_string(zmc_status s);
+ZMC_API int zmc_last_cuda_error(void);          /* cudaError_t of the last ZMC_ERR_CUDA on this thread */
+ZMC_API const char* zmc_version(void);
+/* Validate arguments exactly as zmc_scan_ex does, enqueue nothing; writes G (whole grid) if non-NULL. */
+ZMC_API zmc_status zmc_validate(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                        uint64_t n_samples, const zmc_options* opt, uint64_t* grid_points);
+/* The schedule AUTO would pick for `count` points of `n_samples` samples in N dimensions. */
+ZMC_API int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N);
+/* Batch b of a range cut into batches of batch_points: writes its (first, count). Returns the number of batches. */
+ZMC_API int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_points, int64_t b,
+                        uint64_t* batch_first, uint64_t* batch_count);
+/* Free the cached per-device scratch (staging buffers, streams, events). */
+ZMC_API void zmc_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ZMC_H_ */

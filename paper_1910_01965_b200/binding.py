@@ -1,0 +1,279 @@
+"""Thin ctypes binding of the C ABI in include/zmc.h -- argument marshalling only.
+
+Every step of the hot path (decode, Philox, integrand, reduction, finalise, result streaming)
+runs inside libzmc.so; this module converts Python/numpy/torch arguments to plain pointers and
+sizes.  torch is used for device / pinned memory and streams only.  There is NO fallback: if
+libzmc.so cannot be built or loaded, importing callers get a RuntimeError.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libzmc.so")
+
+# --- mirrors of include/zmc.h ----------------------------------------------------------------
+ZMC_OK, ZMC_ERR_INVALID_ARG, ZMC_ERR_UNKNOWN_INTEGRAND, ZMC_ERR_SHAPE_MISMATCH = 0, 1, 2, 3
+ZMC_ERR_GRID_TOO_LARGE, ZMC_ERR_OUT_OF_MEMORY, ZMC_ERR_CUDA = 4, 5, 6
+ZMC_PREC_F64, ZMC_PREC_F32E = 0, 1
+ZMC_OUT_F64, ZMC_OUT_F32 = 0, 1
+ZMC_LOC_DEVICE, ZMC_LOC_HOST = 0, 1
+ZMC_SCHED_AUTO, ZMC_SCHED_THREAD, ZMC_SCHED_WARP, ZMC_SCHED_CTA = 0, 1, 2, 3
+ZMC_FAST_MATH_DEFAULT, ZMC_FAST_MATH_OFF, ZMC_FAST_MATH_ON = -1, 0, 1
+
+EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info_at",
+           "zmc_integrand_info_by_id", "zmc_status_string", "zmc_last_cuda_error", "zmc_version",
+           "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown"]
+
+
+class zmc_param_list(ctypes.Structure):
+    _fields_ = [("values", ctypes.POINTER(ctypes.c_double)), ("count", ctypes.c_int64)]
+
+
+class zmc_options(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_uint32), ("precision", ctypes.c_int32), ("out_dtype", ctypes.c_int32),
+                ("out_location", ctypes.c_int32), ("schedule", ctypes.c_int32), ("fast_math", ctypes.c_int32),
+                ("batch_points", ctypes.c_uint64), ("first_index", ctypes.c_uint64), ("count", ctypes.c_uint64),
+                ("consts", ctypes.POINTER(ctypes.c_double)), ("n_consts", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
+
+
+class zmc_timing(ctypes.Structure):
+    _fields_ = [("h2d_ms", ctypes.c_double), ("kernel_ms", ctypes.c_double), ("d2h_ms", ctypes.c_double),
+                ("exposed_d2h_ms", ctypes.c_double), ("wall_ms", ctypes.c_double), ("n_batches", ctypes.c_int64),
+                ("gpu_launches", ctypes.c_int64), ("d2h_bytes", ctypes.c_uint64), ("h2d_bytes", ctypes.c_uint64),
+                ("schedule", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+    def as_dict(self):
+        return {f: getattr(self, f) for f, _ in self._fields_ if f != "reserved"}
+
+
+class zmc_integrand_info(ctypes.Structure):
+    _fields_ = [("id", ctypes.c_int32), ("name", ctypes.c_char_p), ("N_min", ctypes.c_int32),
+                ("N_max", ctypes.c_int32), ("M_min", ctypes.c_int32), ("M_max", ctypes.c_int32),
+                ("n_consts", ctypes.c_int32), ("has_closed_form", ctypes.c_int32)]
+
+
+class ZmcError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"zmc status {status}: {message}")
+        self.status = status
+
+
+_lib = None
+
+
+def load():
+    """Load libzmc.so (building it with nvcc if it is missing).  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as exc:  # noqa: BLE001
+            raise RuntimeError(f"libzmc.so is missing and could not be built ({exc}); "
+                               "run `python -m paper_1910_01965_b200.build` -- there is no CPU fallback") from exc
+    lib = ctypes.CDLL(LIB_PATH)
+    P = ctypes.POINTER
+    scan_args = [ctypes.c_int, ctypes.c_int, P(ctypes.c_double), ctypes.c_int, P(zmc_param_list),
+                 ctypes.c_uint64, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    lib.zmc_scan.argtypes = scan_args
+    lib.zmc_scan.restype = ctypes.c_int
+    lib.zmc_scan_ex.argtypes = scan_args + [P(zmc_options), P(zmc_timing)]
+    lib.zmc_scan_ex.restype = ctypes.c_int
+    lib.zmc_integrand_count.restype = ctypes.c_int
+    lib.zmc_integrand_info_at.argtypes = [ctypes.c_int, P(zmc_integrand_info)]
+    lib.zmc_integrand_info_by_id.argtypes = [ctypes.c_int, P(zmc_integrand_info)]
+    lib.zmc_status_string.argtypes = [ctypes.c_int]
+    lib.zmc_status_string.restype = ctypes.c_char_p
+    lib.zmc_last_cuda_error.restype = ctypes.c_int
+    lib.zmc_version.restype = ctypes.c_char_p
+    lib.zmc_validate.argtypes = [ctypes.c_int, ctypes.c_int, P(ctypes.c_double), ctypes.c_int, P(zmc_param_list),
+                                 ctypes.c_uint64, P(zmc_options), P(ctypes.c_uint64)]
+    lib.zmc_validate.restype = ctypes.c_int
+    lib.zmc_pick_schedule.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int]
+    lib.zmc_pick_schedule.restype = ctypes.c_int
+    lib.zmc_batch_range.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int64,
+                                    P(ctypes.c_uint64), P(ctypes.c_uint64)]
+    lib.zmc_batch_range.restype = ctypes.c_int64
+    lib.zmc_shutdown.restype = None
+    _lib = lib
+    return lib
+
+
+def _check(status: int):
+    if status != ZMC_OK:
+        lib = load()
+        msg = lib.zmc_status_string(status).decode()
+        if status == ZMC_ERR_CUDA:
+            msg += f" (cudaError {lib.zmc_last_cuda_error()})"
+        raise ZmcError(status, msg)
+
+
+class _Marshalled:
+    """Keeps the numpy buffers alive while the C call reads them."""
+
+    def __init__(self, bounds, lists, consts):
+        self.bounds = np.ascontiguousarray(bounds, dtype=np.float64)
+        self.lists = [np.ascontiguousarray(l, dtype=np.float64) for l in lists]
+        self.c_lists = (zmc_param_list * max(len(self.lists), 1))()
+        for i, l in enumerate(self.lists):
+            self.c_lists[i].values = l.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+            self.c_lists[i].count = len(l)
+        self.consts = np.ascontiguousarray(consts if consts is not None else [], dtype=np.float64)
+
+    @property
+    def N(self):
+        return len(self.bounds) // 2
+
+    @property
+    def M(self):
+        return len(self.lists)
+
+    def bounds_ptr(self):
+        return self.bounds.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+    def consts_ptr(self):
+        return self.consts.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if len(self.consts) else None
+
+
+def _make_options(m: _Marshalled, precision, out_dtype, out_location, schedule, fast_math, batch_points,
+                  first_index, count) -> zmc_options:
+    o = zmc_options()
+    o.struct_size = ctypes.sizeof(zmc_options)
+    o.precision, o.out_dtype, o.out_location = precision, out_dtype, out_location
+    o.schedule, o.fast_math = schedule, fast_math
+    o.batch_points, o.first_index, o.count = batch_points, first_index, count
+    o.consts = m.consts_ptr()
+    o.n_consts = len(m.consts)
+    return o
+
+
+def _tensor_ptr(t):
+    """(pointer, out_dtype, out_location) of a torch tensor (cuda or pinned/pageable cpu) or numpy array."""
+    if isinstance(t, np.ndarray):
+        dt = {np.dtype(np.float64): ZMC_OUT_F64, np.dtype(np.float32): ZMC_OUT_F32}[t.dtype]
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data, dt, ZMC_LOC_HOST
+    import torch
+    assert t.is_contiguous()
+    dt = {torch.float64: ZMC_OUT_F64, torch.float32: ZMC_OUT_F32}[t.dtype]
+    return t.data_ptr(), dt, (ZMC_LOC_DEVICE if t.is_cuda else ZMC_LOC_HOST)
+
+
+def _stream_handle(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def zmc_scan(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, stream=None):
+    """include/zmc.h zmc_scan: fp64 path, double device outputs, one batch, AUTO schedule."""
+    m = _Marshalled(bounds, lists, None)
+    pm, dm, lm = _tensor_ptr(out_mean)
+    pe, de, le = _tensor_ptr(out_stderr)
+    if (dm, lm, de, le) != (ZMC_OUT_F64, ZMC_LOC_DEVICE, ZMC_OUT_F64, ZMC_LOC_DEVICE):
+        raise ZmcError(ZMC_ERR_INVALID_ARG, "zmc_scan writes float64 CUDA tensors; use zmc_scan_ex otherwise")
+    _check(load().zmc_scan(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_samples, seed,
+                           ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(_stream_handle(stream))))
+
+
+def zmc_scan_ex(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, stream=None, *,
+                precision: int = ZMC_PREC_F64, schedule: int = ZMC_SCHED_AUTO,
+                fast_math: int = ZMC_FAST_MATH_DEFAULT, batch_points: int = 0, first_index: int = 0,
+                count: int = 0, consts=None, timing: bool = False) -> Optional[dict]:
+    """include/zmc.h zmc_scan_ex.  Output dtype/location are taken from the output tensors
+    (torch CUDA tensor = DEVICE; torch CPU tensor or numpy array = HOST).  Returns the timing
+    dict when timing=True (the call then synchronises), else None."""
+    m = _Marshalled(bounds, lists, consts)
+    pm, dm, lm = _tensor_ptr(out_mean)
+    pe, de, le = _tensor_ptr(out_stderr)
+    if (dm, lm) != (de, le):
+        raise ZmcError(ZMC_ERR_INVALID_ARG, "out_mean and out_stderr must share dtype and location")
+    o = _make_options(m, precision, dm, lm, schedule, fast_math, batch_points, first_index, count)
+    tm = zmc_timing() if timing else None
+    _check(load().zmc_scan_ex(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_samples, seed,
+                              ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(_stream_handle(stream)),
+                              ctypes.byref(o), ctypes.byref(tm) if timing else None))
+    return tm.as_dict() if timing else None
+
+
+def zmc_validate(integrand_id: int, bounds, lists, n_samples: int, *, precision: int = ZMC_PREC_F64,
+                 first_index: int = 0, count: int = 0, consts=None, schedule: int = ZMC_SCHED_AUTO,
+                 out_dtype: int = ZMC_OUT_F64, out_location: int = ZMC_LOC_DEVICE,
+                 fast_math: int = ZMC_FAST_MATH_DEFAULT, batch_points: int = 0):
+    """Returns (status, grid_points) without raising and without touching a GPU."""
+    m = _Marshalled(bounds, lists, consts)
+    o = _make_options(m, precision, out_dtype, out_location, schedule, fast_math, batch_points, first_index, count)
+    g = ctypes.c_uint64(0)
+    st = load().zmc_validate(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_samples, ctypes.byref(o),
+                             ctypes.byref(g))
+    return int(st), int(g.value)
+
+
+def zmc_pick_schedule(count: int, n_samples: int, N: int) -> int:
+    return int(load().zmc_pick_schedule(count, n_samples, N))
+
+
+def zmc_batch_range(first_index: int, count: int, batch_points: int, b: int):
+    """Returns (n_batches, batch_first, batch_count) of batch b."""
+    f, c = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    nb = load().zmc_batch_range(first_index, count, batch_points, b, ctypes.byref(f), ctypes.byref(c))
+    return int(nb), int(f.value), int(c.value)
+
+
+def zmc_integrands():
+    lib = load()
+    out = []
+    for i in range(lib.zmc_integrand_count()):
+        info = zmc_integrand_info()
+        _check(lib.zmc_integrand_info_at(i, ctypes.byref(info)))
+        out.append({"id": info.id, "name": info.name.decode(), "N": (info.N_min, info.N_max),
+                    "M": (info.M_min, info.M_max), "n_consts": info.n_consts,
+                    "has_closed_form": bool(info.has_closed_form)})
+    return out
+
+
+def zmc_version() -> str:
+    return load().zmc_version().decode()
+
+
+def zmc_status_string(status: int) -> str:
+    return load().zmc_status_string(status).decode()
+
+
+def zmc_shutdown():
+    load().zmc_shutdown()
+
+
+def scan_workload(w, *, schedule: int = ZMC_SCHED_AUTO, fast_math: int = ZMC_FAST_MATH_DEFAULT,
+                  first_index: int = 0, count: int = 0, batch_points: Optional[int] = None,
+                  host_out: Optional[bool] = None, out_mean=None, out_stderr=None, timing: bool = False,
+                  stream=None):
+    """Convenience for tests/bench: run a workloads.Workload; allocates the outputs (torch) unless given.
+    Returns (out_mean, out_stderr, timing_dict_or_None); outputs are valid after the stream is synchronised."""
+    import torch
+    n_out = count if count else w.G - first_index
+    dtype = torch.float32 if w.out_f32 else torch.float64
+    host = w.host_out if host_out is None else host_out
+    if out_mean is None:
+        if host:
+            out_mean = torch.empty(n_out, dtype=dtype, pin_memory=True)
+            out_stderr = torch.empty(n_out, dtype=dtype, pin_memory=True)
+        else:
+            out_mean = torch.empty(n_out, dtype=dtype, device="cuda")
+            out_stderr = torch.empty(n_out, dtype=dtype, device="cuda")
+    tm = zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, out_mean, out_stderr, stream,
+                     precision=w.precision, schedule=schedule, fast_math=fast_math,
+                     batch_points=w.batch_points if batch_points is None else batch_points,
+                     first_index=first_index, count=count, consts=w.consts, timing=timing)
+    return out_mean, out_stderr, tm

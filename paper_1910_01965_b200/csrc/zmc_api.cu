@@ -1,0 +1,490 @@
+// zmc_api.cu -- the C ABI of include/zmc.h: argument validation (H1), the batch scheduler (H2),
+// kernel dispatch, and result streaming to host memory on a side stream (H8).
+//
+// PAPER.md:65 "we cut the parameter grid into several batches. Each batch is fed into one GPU
+// device for evaluation"; PAPER.md:85, :132-140 report HToD, DToH and GPU evaluation time
+// separately -- zmc_timing keeps that split.  There is no CPU fallback anywhere in this file.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "zmc_params.h"
+
+namespace zmc {
+extern const KernelEntry kEntriesC12[];  extern const int kNumEntriesC12;
+extern const KernelEntry kEntriesC3[];   extern const int kNumEntriesC3;
+extern const KernelEntry kEntriesC45[];  extern const int kNumEntriesC45;
+extern const KernelEntry kEntriesP6[];   extern const int kNumEntriesP6;
+extern const KernelEntry kEntriesDiag[]; extern const int kNumEntriesDiag;
+}  // namespace zmc
+
+using namespace zmc;
+
+namespace {
+
+const zmc_integrand_info kFamilies[] = {
+    {ZMC_FAM_C1_COS_XY, "c1_cos_xy", 1, 1, 1, 1, 0, 1},
+    {ZMC_FAM_C2_SIN_XY2, "c2_sin_xy2", 2, 2, 2, 2, 0, 1},
+    {ZMC_FAM_C3_OSCILLATORY, "c3_oscillatory", 1, ZMC_MAX_N, 3, 3, 1, 1},
+    {ZMC_FAM_C4_GAUSS_PEAK, "c4_gauss_peak", 6, 6, 4, 4, 0, 1},
+    {ZMC_FAM_C5_DAMPED_COS, "c5_damped_cos", 3, 3, 5, 5, 0, 1},
+    {ZMC_FAM_P6_SIN_SUM, "p6_sin_sum", 1, ZMC_MAX_N, 1, ZMC_MAX_M, 0, 1},
+    {ZMC_FAM_CONST_ONE, "const_one", 1, ZMC_MAX_N, 1, ZMC_MAX_M, 0, 1},
+    {ZMC_FAM_PARAM_ECHO, "param_echo", 1, ZMC_MAX_N, 1, ZMC_MAX_M, 1, 1},
+    {ZMC_FAM_LIN_Y, "lin_y", 1, ZMC_MAX_N, 1, ZMC_MAX_M, 1, 1},
+    {ZMC_FAM_POLY, "poly", 1, ZMC_MAX_N, 1, ZMC_MAX_M, 0, 1},
+};
+const int kNumFamilies = sizeof(kFamilies) / sizeof(kFamilies[0]);
+
+thread_local int tl_cuda_error = 0;
+
+zmc_status cuda_fail(cudaError_t e) {
+    tl_cuda_error = (int)e;
+    return (e == cudaErrorMemoryAllocation) ? ZMC_ERR_OUT_OF_MEMORY : ZMC_ERR_CUDA;
+}
+#define ZMC_CUDA(call)                                   \
+    do {                                                 \
+        cudaError_t e__ = (call);                        \
+        if (e__ != cudaSuccess) return cuda_fail(e__);   \
+    } while (0)
+
+const zmc_integrand_info* find_family(int id) {
+    for (int i = 0; i < kNumFamilies; ++i)
+        if (kFamilies[i].id == id) return &kFamilies[i];
+    return nullptr;
+}
+
+struct Options {     // zmc_options with defaults applied
+    int precision = ZMC_PREC_F64, out_dtype = ZMC_OUT_F64, out_location = ZMC_LOC_DEVICE;
+    int schedule = ZMC_SCHED_AUTO, fast_math = ZMC_FAST_MATH_DEFAULT;
+    uint64_t batch_points = 0, first_index = 0, count = 0;
+    const double* consts = nullptr;
+    int n_consts = 0;
+};
+
+zmc_status read_options(const zmc_options* o, Options* out) {
+    if (!o) return ZMC_OK;
+    if (o->struct_size < sizeof(zmc_options)) return ZMC_ERR_INVALID_ARG;
+    out->precision = o->precision;
+    out->out_dtype = o->out_dtype;
+    out->out_location = o->out_location;
+    out->schedule = o->schedule;
+    out->fast_math = o->fast_math;
+    out->batch_points = o->batch_points;
+    out->first_index = o->first_index;
+    out->count = o->count;
+    out->consts = o->consts;
+    out->n_consts = o->n_consts;
+    if (out->precision != ZMC_PREC_F64 && out->precision != ZMC_PREC_F32E) return ZMC_ERR_INVALID_ARG;
+    if (out->out_dtype != ZMC_OUT_F64 && out->out_dtype != ZMC_OUT_F32) return ZMC_ERR_INVALID_ARG;
+    if (out->out_location != ZMC_LOC_DEVICE && out->out_location != ZMC_LOC_HOST) return ZMC_ERR_INVALID_ARG;
+    if (out->schedule < ZMC_SCHED_AUTO || out->schedule > ZMC_SCHED_CTA) return ZMC_ERR_INVALID_ARG;
+    if (out->fast_math < ZMC_FAST_MATH_DEFAULT || out->fast_math > ZMC_FAST_MATH_ON) return ZMC_ERR_INVALID_ARG;
+    if (out->n_consts < 0 || out->n_consts > ZMC_MAX_CONSTS) return ZMC_ERR_INVALID_ARG;
+    if (out->n_consts > 0 && !out->consts) return ZMC_ERR_INVALID_ARG;
+    return ZMC_OK;
+}
+
+// All argument checks (reading Q18).  Nothing is enqueued and no output is touched on failure.
+zmc_status validate(int id, int N, const double* bounds, int M, const zmc_param_list* lists, uint64_t n_samples,
+                    const Options& o, uint64_t* G_out, uint64_t* first_out, uint64_t* count_out) {
+    if (!bounds || !lists) return ZMC_ERR_INVALID_ARG;
+    if (N < 1 || N > ZMC_MAX_N || M < 1 || M > ZMC_MAX_M) return ZMC_ERR_INVALID_ARG;
+    if (n_samples < 2 || n_samples > 0xFFFFFFFFull) return ZMC_ERR_INVALID_ARG;
+    if (n_samples * (uint64_t)N > (1ull << 34)) return ZMC_ERR_INVALID_ARG;   // block index stays 32-bit
+    for (int k = 0; k < N; ++k) {
+        const double a = bounds[2 * k], b = bounds[2 * k + 1];
+        if (!std::isfinite(a) || !std::isfinite(b) || !(a < b)) return ZMC_ERR_INVALID_ARG;
+    }
+    uint64_t G = 1;
+    for (int i = 0; i < M; ++i) {
+        if (lists[i].count < 1 || !lists[i].values) return ZMC_ERR_INVALID_ARG;
+        if (lists[i].count > 0x7FFFFFFFll) return ZMC_ERR_GRID_TOO_LARGE;
+        for (int64_t j = 0; j < lists[i].count; ++j)
+            if (!std::isfinite(lists[i].values[j])) return ZMC_ERR_INVALID_ARG;
+        if ((uint64_t)lists[i].count > (1ull << 48) / G) return ZMC_ERR_GRID_TOO_LARGE;
+        G *= (uint64_t)lists[i].count;
+    }
+    for (int c = 0; c < o.n_consts; ++c)
+        if (!std::isfinite(o.consts[c])) return ZMC_ERR_INVALID_ARG;
+    const zmc_integrand_info* fam = find_family(id);
+    if (!fam) return ZMC_ERR_UNKNOWN_INTEGRAND;
+    if (N < fam->N_min || N > fam->N_max || M < fam->M_min || M > fam->M_max || o.n_consts != fam->n_consts)
+        return ZMC_ERR_SHAPE_MISMATCH;
+    if (id == ZMC_FAM_PARAM_ECHO || id == ZMC_FAM_LIN_Y) {
+        const double c = o.consts[0];
+        const int lim = (id == ZMC_FAM_PARAM_ECHO) ? M : N;
+        if (c < 0 || c >= lim || c != std::floor(c)) return ZMC_ERR_SHAPE_MISMATCH;
+    }
+    if (o.first_index > G) return ZMC_ERR_INVALID_ARG;
+    uint64_t count = o.count ? o.count : G - o.first_index;
+    if (count > G - o.first_index) return ZMC_ERR_INVALID_ARG;
+    if (G_out) *G_out = G;
+    if (first_out) *first_out = o.first_index;
+    if (count_out) *count_out = count;
+    return ZMC_OK;
+}
+
+// ---- per-device scratch: side stream, list staging ring, double-buffered result staging ----------
+constexpr int kRing = 4;
+struct ListSlot {
+    double* host = nullptr;      // pinned
+    double* dev = nullptr;
+    size_t cap = 0;              // entries
+    cudaEvent_t done = nullptr;  // last kernel that read `dev`
+    bool used = false;
+};
+struct DeviceScratch {
+    bool init = false;
+    int sm_count = 0;
+    cudaStream_t side = nullptr;
+    ListSlot ring[kRing];
+    int ring_next = 0;
+    void* stage[2] = {nullptr, nullptr};     // result staging (mean then stderr), host-output mode
+    size_t stage_cap = 0;                    // bytes each
+    cudaEvent_t stage_free[2] = {nullptr, nullptr};   // last copy out of stage[i]
+    bool stage_used[2] = {false, false};
+    cudaEvent_t kernel_done[2] = {nullptr, nullptr};
+};
+constexpr int kMaxDevices = 64;
+DeviceScratch g_scratch[kMaxDevices];
+std::mutex g_mutex;
+
+zmc_status get_scratch(int dev, DeviceScratch** out) {
+    if (dev < 0 || dev >= kMaxDevices) return ZMC_ERR_CUDA;
+    DeviceScratch& s = g_scratch[dev];
+    if (!s.init) {
+        ZMC_CUDA(cudaDeviceGetAttribute(&s.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        ZMC_CUDA(cudaStreamCreateWithFlags(&s.side, cudaStreamNonBlocking));
+        for (int i = 0; i < kRing; ++i) ZMC_CUDA(cudaEventCreateWithFlags(&s.ring[i].done, cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) {
+            ZMC_CUDA(cudaEventCreateWithFlags(&s.stage_free[i], cudaEventDisableTiming));
+            ZMC_CUDA(cudaEventCreateWithFlags(&s.kernel_done[i], cudaEventDisableTiming));
+        }
+        s.init = true;
+    }
+    *out = &s;
+    return ZMC_OK;
+}
+
+void free_scratch(DeviceScratch& s) {
+    if (!s.init) return;
+    for (int i = 0; i < kRing; ++i) {
+        if (s.ring[i].host) cudaFreeHost(s.ring[i].host);
+        if (s.ring[i].dev) cudaFree(s.ring[i].dev);
+        if (s.ring[i].done) cudaEventDestroy(s.ring[i].done);
+    }
+    for (int i = 0; i < 2; ++i) {
+        if (s.stage[i]) cudaFree(s.stage[i]);
+        if (s.stage_free[i]) cudaEventDestroy(s.stage_free[i]);
+        if (s.kernel_done[i]) cudaEventDestroy(s.kernel_done[i]);
+    }
+    if (s.side) cudaStreamDestroy(s.side);
+    s = DeviceScratch();
+}
+
+const KernelEntry* find_kernel(int family, int N, int precision, int fast, int schedule) {
+    const KernelEntry* tables[] = {kEntriesC12, kEntriesC3, kEntriesC45, kEntriesP6, kEntriesDiag};
+    const int sizes[] = {kNumEntriesC12, kNumEntriesC3, kNumEntriesC45, kNumEntriesP6, kNumEntriesDiag};
+    const KernelEntry* generic = nullptr;
+    for (int t = 0; t < 5; ++t) {
+        for (int i = 0; i < sizes[t]; ++i) {
+            const KernelEntry& e = tables[t][i];
+            if (e.family != family || e.precision != precision || e.schedule != schedule) continue;
+            if (precision == ZMC_PREC_F32E && e.fast != fast && family < ZMC_FAM_CONST_ONE) continue;
+            if (e.n_dim == N) return &e;
+            if (e.n_dim == 0) generic = &e;
+        }
+    }
+    return generic;
+}
+
+struct TimedSpan { cudaEvent_t a = nullptr, b = nullptr; };
+
+}  // namespace
+
+// --------------------------------------------------------------------------------------------------
+extern "C" {
+
+int zmc_integrand_count(void) { return kNumFamilies; }
+
+zmc_status zmc_integrand_info_at(int index, zmc_integrand_info* info) {
+    if (!info || index < 0 || index >= kNumFamilies) return ZMC_ERR_INVALID_ARG;
+    *info = kFamilies[index];
+    return ZMC_OK;
+}
+
+zmc_status zmc_integrand_info_by_id(int integrand_id, zmc_integrand_info* info) {
+    if (!info) return ZMC_ERR_INVALID_ARG;
+    const zmc_integrand_info* f = find_family(integrand_id);
+    if (!f) return ZMC_ERR_UNKNOWN_INTEGRAND;
+    *info = *f;
+    return ZMC_OK;
+}
+
+const char* zmc_status_string(zmc_status s) {
+    switch (s) {
+        case ZMC_OK: return "ok";
+        case ZMC_ERR_INVALID_ARG: return "invalid argument";
+        case ZMC_ERR_UNKNOWN_INTEGRAND: return "unknown integrand id";
+        case ZMC_ERR_SHAPE_MISMATCH: return "(N, M, n_consts) not accepted by this integrand family";
+        case ZMC_ERR_GRID_TOO_LARGE: return "parameter grid too large";
+        case ZMC_ERR_OUT_OF_MEMORY: return "out of memory";
+        case ZMC_ERR_CUDA: return "CUDA error (see zmc_last_cuda_error)";
+    }
+    return "unknown status";
+}
+
+int zmc_last_cuda_error(void) { return tl_cuda_error; }
+
+const char* zmc_version(void) { return "zmc_scan 0.1 (sm_100a)"; }
+
+zmc_status zmc_validate(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                        uint64_t n_samples, const zmc_options* opt, uint64_t* grid_points) {
+    Options o;
+    zmc_status st = read_options(opt, &o);
+    if (st != ZMC_OK) return st;
+    return validate(integrand_id, N, bounds, M, lists, n_samples, o, grid_points, nullptr, nullptr);
+}
+
+// H6 schedule choice.  R = threads a B200 keeps resident at 4 CTAs/SM (148*1024).  THREAD needs
+// enough points for >= 16 rounds of R (tail <= 6 %); WARP the same in warps; else CTA.  A point
+// with few sample groups cannot feed 32 / 256 lanes, so small n falls back to fewer lanes.
+int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N) {
+    const uint64_t resident = 148ull * 1024ull;
+    const int g4 = (N % 4 == 0) ? 4 : (N % 2 == 0) ? 2 : 1;
+    const uint64_t groups = n_samples / (uint64_t)(4 / g4) + 1;
+    if (count >= 16 * resident || groups < 4 * 32) return ZMC_SCHED_THREAD;
+    if (count >= 16 * (resident / 32) || groups < 4 * 256) return ZMC_SCHED_WARP;
+    return ZMC_SCHED_CTA;
+}
+
+int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_points, int64_t b,
+                        uint64_t* batch_first, uint64_t* batch_count) {
+    if (batch_points == 0 || batch_points > count) batch_points = count;
+    const int64_t nb = count ? (int64_t)((count + batch_points - 1) / batch_points) : 0;
+    if (b >= 0 && b < nb) {
+        const uint64_t f = first_index + (uint64_t)b * batch_points;
+        const uint64_t c = ((uint64_t)b == (uint64_t)nb - 1) ? first_index + count - f : batch_points;
+        if (batch_first) *batch_first = f;
+        if (batch_count) *batch_count = c;
+    }
+    return nb;
+}
+
+void zmc_shutdown(void) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    int cur = 0;
+    const bool have = cudaGetDevice(&cur) == cudaSuccess;
+    for (int d = 0; d < kMaxDevices; ++d) {
+        if (!g_scratch[d].init) continue;
+        if (have) cudaSetDevice(d);
+        free_scratch(g_scratch[d]);
+    }
+    if (have) cudaSetDevice(cur);
+}
+
+zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                    uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream) {
+    return zmc_scan_ex(integrand_id, N, bounds, M, lists, n_samples, seed, out_mean, out_stderr, stream,
+                       nullptr, nullptr);
+}
+
+zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                       uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream_v,
+                       const zmc_options* opt, zmc_timing* timing) {
+    // ---- H1: validate -----------------------------------------------------------------------
+    Options o;
+    zmc_status st = read_options(opt, &o);
+    if (st != ZMC_OK) return st;
+    uint64_t G = 0, first = 0, count = 0;
+    st = validate(integrand_id, N, bounds, M, lists, n_samples, o, &G, &first, &count);
+    if (st != ZMC_OK) return st;
+    if (!out_mean || !out_stderr) return ZMC_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    if (timing) std::memset(timing, 0, sizeof(*timing));
+
+    const bool f32e = o.precision == ZMC_PREC_F32E;
+    const int fast = f32e ? (o.fast_math == ZMC_FAST_MATH_OFF ? 0 : 1) : 0;
+    const int schedule = o.schedule == ZMC_SCHED_AUTO ? zmc_pick_schedule(count, n_samples, N) : o.schedule;
+    const KernelEntry* kern = find_kernel(integrand_id, N, o.precision, fast, schedule);
+    if (!kern) return ZMC_ERR_UNKNOWN_INTEGRAND;
+    if (timing) timing->schedule = schedule;
+    if (count == 0) return ZMC_OK;
+
+    std::lock_guard<std::mutex> lock(g_mutex);
+    int dev = 0;
+    ZMC_CUDA(cudaGetDevice(&dev));
+    DeviceScratch* s = nullptr;
+    st = get_scratch(dev, &s);
+    if (st != ZMC_OK) return st;
+
+    // ---- parameter block -----------------------------------------------------------------------
+    ScanParams p;
+    std::memset(&p, 0, sizeof(p));
+    auto mirror = [f32e](double v) { return f32e ? (double)(float)v : v; };
+    p.n = (uint32_t)n_samples;
+    p.n_dim = (uint32_t)N;
+    p.n_par = (uint32_t)M;
+    p.out_f32 = o.out_dtype == ZMC_OUT_F32;
+    p.volume = 1.0;
+    for (int k = 0; k < N; ++k) {
+        p.a[k] = mirror(bounds[2 * k]);
+        p.width[k] = mirror(bounds[2 * k + 1] - bounds[2 * k]);
+        p.volume *= p.width[k];
+    }
+    for (int c = 0; c < o.n_consts; ++c) p.consts[c] = mirror(o.consts[c]);
+    {
+        uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+        for (int r = 0; r < 10; ++r) {
+            p.rk[2 * r] = k0;
+            p.rk[2 * r + 1] = k1;
+            k0 += 0x9E3779B9u;
+            k1 += 0xBB67AE85u;
+        }
+    }
+    size_t total = 0;
+    for (int i = 0; i < M; ++i) {
+        p.counts[i] = (uint32_t)lists[i].count;
+        p.list_off[i] = (uint32_t)total;
+        total += (size_t)lists[i].count;
+    }
+    if (total > 0xFFFFFFFFull) return ZMC_ERR_GRID_TOO_LARGE;
+    p.lists_total = (uint32_t)total;
+    const size_t elem_eval = f32e ? 4 : 8;
+    // shared-memory staging pays off when a CTA serves many points (THREAD schedule) and the lists fit
+    const size_t smem_bytes = (schedule == ZMC_SCHED_THREAD && total * elem_eval <= 48 * 1024) ? total * elem_eval : 0;
+    p.stage_smem = smem_bytes ? 1u : 0u;
+
+    // ---- H1: stage the lists (pinned ring slot -> device) ------------------------------------------
+    ListSlot& slot = s->ring[s->ring_next];
+    s->ring_next = (s->ring_next + 1) % kRing;
+    if (slot.used) ZMC_CUDA(cudaEventSynchronize(slot.done));
+    if (slot.cap < total) {
+        if (slot.host) cudaFreeHost(slot.host);
+        if (slot.dev) cudaFree(slot.dev);
+        slot.host = nullptr; slot.dev = nullptr; slot.cap = 0;
+        ZMC_CUDA(cudaMallocHost(&slot.host, total * sizeof(double)));
+        ZMC_CUDA(cudaMalloc(&slot.dev, total * sizeof(double)));
+        slot.cap = total;
+    }
+    for (int i = 0; i < M; ++i)
+        std::memcpy(slot.host + p.list_off[i], lists[i].values, (size_t)lists[i].count * sizeof(double));
+    p.lists = slot.dev;
+
+    std::vector<cudaEvent_t> tev;          // timing events, destroyed before return
+    auto new_tev = [&tev](cudaEvent_t* e) -> cudaError_t {
+        cudaError_t err = cudaEventCreate(e);
+        if (err == cudaSuccess) tev.push_back(*e);
+        return err;
+    };
+    struct Cleanup { std::vector<cudaEvent_t>& v; ~Cleanup() { for (auto e : v) cudaEventDestroy(e); } } cleanup{tev};
+
+    cudaEvent_t ev_begin = nullptr, ev_h2d = nullptr, ev_end = nullptr;
+    if (timing) {
+        ZMC_CUDA(new_tev(&ev_begin)); ZMC_CUDA(new_tev(&ev_h2d)); ZMC_CUDA(new_tev(&ev_end));
+        ZMC_CUDA(cudaEventRecord(ev_begin, stream));
+    }
+    ZMC_CUDA(cudaMemcpyAsync(slot.dev, slot.host, total * sizeof(double), cudaMemcpyHostToDevice, stream));
+    if (timing) ZMC_CUDA(cudaEventRecord(ev_h2d, stream));
+
+    // ---- H2: batches ----------------------------------------------------------------------------------
+    const bool host_out = o.out_location == ZMC_LOC_HOST;
+    const size_t elem_out = p.out_f32 ? 4 : 8;
+    const int64_t n_batches = zmc_batch_range(first, count, o.batch_points, -1, nullptr, nullptr);
+    uint64_t batch_max = (o.batch_points == 0 || o.batch_points > count) ? count : o.batch_points;
+    if (host_out) {
+        const size_t need = (size_t)batch_max * elem_out * 2;
+        if (s->stage_cap < need) {
+            ZMC_CUDA(cudaDeviceSynchronize());          // buffers may still be in flight
+            for (int i = 0; i < 2; ++i) { if (s->stage[i]) cudaFree(s->stage[i]); s->stage[i] = nullptr; }
+            s->stage_cap = 0; s->stage_used[0] = s->stage_used[1] = false;
+            ZMC_CUDA(cudaMalloc(&s->stage[0], need));
+            s->stage_cap = need;
+        }
+        if (n_batches > 1 && !s->stage[1]) ZMC_CUDA(cudaMalloc(&s->stage[1], s->stage_cap));
+    }
+
+    int occ = 0;
+    ZMC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern->func, kThreads, smem_bytes));
+    if (occ < 1) occ = 1;
+    const uint64_t max_grid = (uint64_t)occ * (uint64_t)s->sm_count;
+
+    std::vector<TimedSpan> t_kernel, t_copy;
+    int64_t launches = 0;
+    uint64_t d2h_bytes = 0;
+    for (int64_t b = 0; b < n_batches; ++b) {
+        uint64_t bf = 0, bc = 0;
+        zmc_batch_range(first, count, o.batch_points, b, &bf, &bc);
+        const uint64_t per_cta = schedule == ZMC_SCHED_THREAD ? kThreads : schedule == ZMC_SCHED_WARP ? kThreads / 32 : 1;
+        uint64_t grid = (bc + per_cta - 1) / per_cta;
+        if (grid > max_grid) grid = max_grid;
+        p.first = bf;
+        p.end = bf + bc;
+        p.stride = grid * per_cta;
+        {   // mixed-radix digits of the stride (top digit unbounded)
+            uint64_t rest = p.stride;
+            for (int i = M - 1; i >= 1; --i) { p.stride_digits[i] = (uint32_t)(rest % p.counts[i]); rest /= p.counts[i]; }
+            p.stride_digits[0] = (uint32_t)(rest > 0xFFFFFFFFull ? 0xFFFFFFFFull : rest);
+        }
+        void *dst_mean, *dst_err;
+        const int buf = (int)(b & 1);
+        if (host_out) {
+            if (s->stage_used[buf]) ZMC_CUDA(cudaStreamWaitEvent(stream, s->stage_free[buf], 0));
+            dst_mean = s->stage[buf];
+            dst_err = static_cast<char*>(s->stage[buf]) + (size_t)batch_max * elem_out;
+            p.out_base = bf;
+        } else {
+            dst_mean = out_mean;
+            dst_err = out_stderr;
+            p.out_base = first;
+        }
+        TimedSpan tk;
+        if (timing) { ZMC_CUDA(new_tev(&tk.a)); ZMC_CUDA(new_tev(&tk.b)); ZMC_CUDA(cudaEventRecord(tk.a, stream)); }
+        ZMC_CUDA(kern->launch(p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
+        ++launches;
+        if (timing) { ZMC_CUDA(cudaEventRecord(tk.b, stream)); t_kernel.push_back(tk); }
+
+        if (host_out) {   // H8: copy batch b on the side stream while batch b+1 computes
+            ZMC_CUDA(cudaEventRecord(s->kernel_done[buf], stream));
+            ZMC_CUDA(cudaStreamWaitEvent(s->side, s->kernel_done[buf], 0));
+            TimedSpan tc;
+            if (timing) { ZMC_CUDA(new_tev(&tc.a)); ZMC_CUDA(new_tev(&tc.b)); ZMC_CUDA(cudaEventRecord(tc.a, s->side)); }
+            const size_t off = (size_t)(bf - first) * elem_out, bytes = (size_t)bc * elem_out;
+            ZMC_CUDA(cudaMemcpyAsync(static_cast<char*>(out_mean) + off, dst_mean, bytes, cudaMemcpyDeviceToHost, s->side));
+            ZMC_CUDA(cudaMemcpyAsync(static_cast<char*>(out_stderr) + off, dst_err, bytes, cudaMemcpyDeviceToHost, s->side));
+            if (timing) { ZMC_CUDA(cudaEventRecord(tc.b, s->side)); t_copy.push_back(tc); }
+            ZMC_CUDA(cudaEventRecord(s->stage_free[buf], s->side));
+            s->stage_used[buf] = true;
+            d2h_bytes += 2 * bytes;
+        }
+    }
+    ZMC_CUDA(cudaEventRecord(slot.done, stream));
+    slot.used = true;
+    if (host_out) {   // join the side stream back into `stream`
+        const int last = (int)((n_batches - 1) & 1);
+        ZMC_CUDA(cudaStreamWaitEvent(stream, s->stage_free[last], 0));
+    }
+
+    if (timing) {
+        ZMC_CUDA(cudaEventRecord(ev_end, stream));
+        ZMC_CUDA(cudaEventSynchronize(ev_end));
+        float ms = 0.f;
+        ZMC_CUDA(cudaEventElapsedTime(&ms, ev_begin, ev_h2d)); timing->h2d_ms = ms;
+        ZMC_CUDA(cudaEventElapsedTime(&ms, ev_begin, ev_end)); timing->wall_ms = ms;
+        for (auto& k : t_kernel) { ZMC_CUDA(cudaEventElapsedTime(&ms, k.a, k.b)); timing->kernel_ms += ms; }
+        for (auto& c : t_copy) { ZMC_CUDA(cudaEventElapsedTime(&ms, c.a, c.b)); timing->d2h_ms += ms; }
+        const double exposed = timing->wall_ms - timing->h2d_ms - timing->kernel_ms;
+        timing->exposed_d2h_ms = host_out ? (exposed > 0 ? exposed : 0.0) : 0.0;
+        timing->n_batches = n_batches;
+        timing->gpu_launches = launches;
+        timing->d2h_bytes = d2h_bytes;
+        timing->h2d_bytes = total * sizeof(double);
+    }
+    return ZMC_OK;
+}
+
+}  // extern "C"

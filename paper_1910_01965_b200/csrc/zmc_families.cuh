@@ -1,0 +1,222 @@
+// zmc_families.cuh -- H5: the compiled-in integrand families g(y; x) (BASELINE.json configs 1-5,
+// the paper's Eq. (2)/(4) PAPER.md:75, :120, and four diagnostics), written for the issue-bound
+// hot loop: each family folds the affine sample map y_k = a_k + width_k*u_k (reading S5) and every
+// per-point factor into constants computed ONCE per grid point in fp64 (setup), so that the
+// per-sample work (eval) is one FMA per dimension plus the family's own arithmetic.
+//
+// Interface:  struct Fam { using real; static constexpr int kN (0 = runtime N);
+//                          void setup(const real* x, const ScanParams& p);   // once per point
+//                          real eval(const uint32_t* w) const; }             // w: the N words of one sample
+#pragma once
+#include <type_traits>
+#include "zmc_math.cuh"
+#include "zmc_params.h"
+
+namespace zmc {
+
+constexpr double kInvPi = 0.31830988618379067154;
+constexpr double kPi = 3.141592653589793;                 // reading S8
+constexpr double kTwoPi = 2.0 * 3.141592653589793;
+constexpr double kSqrtLog2e = 1.2011224087864498;         // sqrt(log2(e))
+constexpr double kLog2e = 1.4426950408889634;
+
+// a'_k = a_k - (1-eps)*width_k : y_k = a'_k + width_k * f_k with f_k = unit(w_k) in [1,2)
+template <typename R> __device__ __forceinline__ double a_fold(const ScanParams& p, int k) {
+    return ::fma(-(double)Real<R>::one_minus_eps(), p.width[k], p.a[k]);
+}
+
+// reduce a phase constant (radians) to [-pi, pi] in fp64 before it is rounded to fp32
+__device__ __forceinline__ double wrap_2pi(double c) { return c - kTwoPi * rint(c * (0.5 * kInvPi)); }
+
+// Trig families share one shape: g = sin(phase), phase = C + sum_k X_k f_k.
+// fp64: phase kept in units of pi (exact range reduction, see sinpi_f64); fp32: radians -> MUFU.
+template <typename R, int N_, bool FAST> struct PhaseSin {
+    using real = R;
+    static constexpr int kN = N_;
+    static constexpr int kMaxN = N_ ? N_ : ZMC_MAX_N;
+    R X[kMaxN];
+    R C;
+    int n_dim;
+
+    // coefficient c_k of y_k and the constant phase c0 (radians); quarter = 1 adds pi/2 (cos)
+    template <class Coef> __device__ __forceinline__ void set(const ScanParams& p, Coef coef, double c0, bool as_cos) {
+        n_dim = N_ ? N_ : (int)p.n_dim;
+        double c = c0;
+#pragma unroll
+        for (int k = 0; k < kMaxN; ++k) {
+            if (k < n_dim) {
+                const double ck = coef(k);
+                c = ::fma(ck, a_fold<R>(p, k), c);
+                if constexpr (std::is_same<R, double>::value) X[k] = ck * p.width[k] * kInvPi;
+                else X[k] = (R)(ck * p.width[k]);
+            }
+        }
+        if constexpr (std::is_same<R, double>::value) C = ::fma(c, kInvPi, as_cos ? 0.5 : 0.0);
+        else C = (R)wrap_2pi(as_cos ? c + 0.5 * kPi : c);
+    }
+
+    __device__ __forceinline__ R phase(const uint32_t* w) const {
+        R ph = C;
+#pragma unroll
+        for (int k = 0; k < kMaxN; ++k)
+            if (k < n_dim) ph = Real<R>::fma(Real<R>::unit(w[k]), X[k], ph);
+        return ph;
+    }
+
+    __device__ __forceinline__ R eval(const uint32_t* w) const {
+        if constexpr (std::is_same<R, double>::value) return sinpi_f64(phase(w));
+        else return Fn<R, FAST>::sin_rad(phase(w));
+    }
+};
+
+// c1: cos(x1*y0)                                                       (BASELINE.json configs[0])
+template <typename R, bool FAST> struct FamC1 : PhaseSin<R, 1, FAST> {
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        const double x1 = (double)x[0];
+        this->set(p, [=](int) { return x1; }, 0.0, true);
+    }
+};
+
+// c2: sin(x1*y0 + x2*y1)                                               (configs[1])
+template <typename R, bool FAST> struct FamC2 : PhaseSin<R, 2, FAST> {
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        const double x1 = (double)x[0], x2 = (double)x[1];
+        this->set(p, [=](int k) { return k == 0 ? x1 : x2; }, 0.0, false);
+    }
+};
+
+// c3: cos(2 pi u + sum_k c_k y_k), c_k = x_{(k mod 3)+1} * (k+1)       (configs[2])
+template <typename R, int N_, bool FAST> struct FamC3 : PhaseSin<R, N_, FAST> {
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        const double x1 = (double)x[0], x2 = (double)x[1], x3 = (double)x[2];
+        this->set(p, [=](int k) { const int m = k % 3; return (m == 0 ? x1 : m == 1 ? x2 : x3) * (double)(k + 1); },
+                  kTwoPi * p.consts[0], true);
+    }
+};
+
+// p6: sin(sum_k y_k + sum_l x_l)                                       (PAPER.md:75 Eq. 2, :120 Eq. 4)
+template <typename R, int N_, bool FAST> struct FamP6 : PhaseSin<R, N_, FAST> {
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        double xs = 0.0;
+#pragma unroll
+        for (int l = 0; l < ZMC_MAX_M; ++l)
+            if (l < (int)p.n_par) xs += (double)x[l];
+        this->set(p, [](int) { return 1.0; }, xs, false);
+    }
+};
+
+// c4: exp(-a^2 sum_k (y_k - w_k)^2), a = x1, w = (x2,x2,x3,x3,x4,x4)   (configs[3])
+// e_k = sqrt(log2 e) * a * (y_k - w_k) = A_k f_k + B_k ; g = 2^-(sum e_k^2): 2 FMA per dimension + one MUFU.EX2
+template <typename R, bool FAST> struct FamC4 {
+    using real = R;
+    static constexpr int kN = 6;
+    R A[6], B[6];
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        const double a = (double)x[0] * kSqrtLog2e;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const double wk = (double)x[1 + (k >> 1)];
+            A[k] = (R)(a * p.width[k]);
+            B[k] = (R)(a * (a_fold<R>(p, k) - wk));
+        }
+    }
+    __device__ __forceinline__ R eval(const uint32_t* w) const {
+        R acc = (R)0;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const R e = Real<R>::fma(Real<R>::unit(w[k]), A[k], B[k]);
+            acc = Real<R>::fma(e, e, acc);
+        }
+        return Fn<R, FAST>::exp2_neg(acc);
+    }
+};
+
+// c5: exp(-x1 |y|^2) cos(x2 y0 + x3 y1 + x4 y2) (1 + x5 y0 y1 y2)      (configs[4])
+template <typename R, bool FAST> struct FamC5 {
+    using real = R;
+    static constexpr int kN = 3;
+    R W[3], Af[3];      // y_k = W_k f_k + Af_k
+    R X[3], C;          // cos phase = C + sum X_k f_k
+    R damp, x5;         // x1 * log2(e)
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        double c = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double af = a_fold<R>(p, k), ck = (double)x[1 + k];
+            W[k] = (R)p.width[k];
+            Af[k] = (R)af;
+            c = ::fma(ck, af, c);
+            if constexpr (std::is_same<R, double>::value) X[k] = ck * p.width[k] * kInvPi;
+            else X[k] = (R)(ck * p.width[k]);
+        }
+        if constexpr (std::is_same<R, double>::value) C = ::fma(c, kInvPi, 0.5);
+        else C = (R)wrap_2pi(c + 0.5 * kPi);
+        damp = (R)((double)x[0] * kLog2e);
+        x5 = x[4];
+    }
+    __device__ __forceinline__ R eval(const uint32_t* w) const {
+        const R f0 = Real<R>::unit(w[0]), f1 = Real<R>::unit(w[1]), f2 = Real<R>::unit(w[2]);
+        const R y0 = Real<R>::fma(f0, W[0], Af[0]);
+        const R y1 = Real<R>::fma(f1, W[1], Af[1]);
+        const R y2 = Real<R>::fma(f2, W[2], Af[2]);
+        const R r2 = Real<R>::fma(y2, y2, Real<R>::fma(y1, y1, y0 * y0));
+        const R ph = Real<R>::fma(f2, X[2], Real<R>::fma(f1, X[1], Real<R>::fma(f0, X[0], C)));
+        const R poly = Real<R>::fma(x5, y0 * y1 * y2, (R)1);
+        R osc;
+        if constexpr (std::is_same<R, double>::value) osc = sinpi_f64(ph);
+        else osc = Fn<R, FAST>::sin_rad(ph);
+        return Fn<R, FAST>::exp2_neg(damp * r2) * osc * poly;
+    }
+};
+
+// ---- diagnostics (tests only): exact y_k = fma(u_k, width_k, a_k), no folding ---------------------
+template <typename R> struct FamConstOne {
+    using real = R;
+    static constexpr int kN = 0;
+    __device__ __forceinline__ void setup(const R*, const ScanParams&) {}
+    __device__ __forceinline__ R eval(const uint32_t*) const { return (R)1; }
+};
+
+template <typename R> struct FamParamEcho {
+    using real = R;
+    static constexpr int kN = 0;
+    R v;
+    __device__ __forceinline__ void setup(const R* x, const ScanParams& p) {
+        const int i = (int)p.consts[0];
+        v = x[0];
+#pragma unroll
+        for (int l = 1; l < ZMC_MAX_M; ++l)
+            if (l == i) v = x[l];
+    }
+    __device__ __forceinline__ R eval(const uint32_t*) const { return v; }
+};
+
+template <typename R> struct FamLinY {
+    using real = R;
+    static constexpr int kN = 0;
+    R a, width;
+    int k;
+    __device__ __forceinline__ void setup(const R*, const ScanParams& p) {
+        k = (int)p.consts[0];
+        a = (R)p.a[k];
+        width = (R)p.width[k];
+    }
+    __device__ __forceinline__ R eval(const uint32_t* w) const {
+        return Real<R>::fma(uniform<R>(w[k]), width, a);
+    }
+};
+
+template <typename R> struct FamPoly {
+    using real = R;
+    static constexpr int kN = 0;
+    const ScanParams* pp;
+    __device__ __forceinline__ void setup(const R*, const ScanParams& p) { pp = &p; }
+    __device__ __forceinline__ R eval(const uint32_t* w) const {
+        R prod = (R)1;
+        for (int k = 0; k < (int)pp->n_dim; ++k)
+            prod *= Real<R>::fma(uniform<R>(w[k]), (R)pp->width[k], (R)pp->a[k]);
+        return prod;
+    }
+};
+
+}  // namespace zmc

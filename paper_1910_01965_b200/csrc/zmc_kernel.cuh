@@ -1,0 +1,246 @@
+// zmc_kernel.cuh -- the fused batch kernel of zmc_scan (sm_100a):
+//   H3 decode -> H4 Philox sampler -> H5 integrand -> H6 fp64 accumulate + reduce -> H7 finalise + store
+// for one contiguous range of flat grid indices (one batch).  One kernel template,
+// three schedules (lanes per grid point): THREAD (1; the paper's mapping), WARP (32)
+// and CTA (256) with __shfl_xor_sync trees -- the paper's one-thread-per-point scheme cannot fill
+// the GPU for small grids and serialises large sample counts.
+//
+// Work split inside a point: samples are taken in block-aligned groups of S samples = NB whole
+// Philox blocks (no random word is wasted, reading S3); lane l of L takes groups l, l+L, ...
+// Every word is keyed by (seed, GLOBAL flat index t, word index), so results are independent of
+// batching and grid size; the summation order (hence the last bits) depends on the schedule only.
+//
+// Accumulation (reading S6): values are shifted by K = g(sample 0 of the point), common to all
+// lanes, and A = sum (g-K), B = sum (g-K)^2 are kept in fp64, so lanes combine by plain addition
+// and  mean = V (K + A/n),  stderr = V sqrt((B - A^2/n) / ((n-1) n))  is free of cancellation.
+#pragma once
+#include "zmc_families.cuh"
+
+namespace zmc {
+
+constexpr int gcd4(int n) { return (n % 4 == 0) ? 4 : (n % 2 == 0) ? 2 : 1; }
+
+// group shape for compile-time N: the smallest block-aligned group, doubled when it is a single block
+template <int N> struct GroupShape {
+    static constexpr int kMinS = 4 / gcd4(N), kMinNB = N / gcd4(N);
+    static constexpr int kU = (kMinNB == 1) ? 2 : 1;
+    static constexpr int S = kMinS * kU, NB = kMinNB * kU;
+};
+template <> struct GroupShape<0> {     // runtime N: 4 samples = N blocks
+    static constexpr int S = 4, NB = ZMC_MAX_N;
+};
+
+template <typename R> struct Accum {
+    double A = 0.0, B = 0.0;
+    R K;
+    __device__ __forceinline__ void add(R g) {
+        double d;
+        if constexpr (std::is_same<R, double>::value) d = g - K;
+        else d = (double)(g - K);          // fp32 subtract is exact when g ~ K (Sterbenz), else harmless
+        A += d;
+        B = ::fma(d, d, B);
+    }
+};
+
+template <class Fam, int SCHED>
+__global__ void __launch_bounds__(kThreads, std::is_same<typename Fam::real, double>::value ? 3 : 4)
+zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mean, void* __restrict__ out_stderr)
+{
+    using R = typename Fam::real;
+    constexpr int kN = Fam::kN;
+    using GS = GroupShape<kN>;
+    constexpr int S = GS::S;
+    const int N = kN ? kN : (int)p.n_dim;
+    const int NB = kN ? GS::NB : N;
+    const int M = (int)p.n_par;
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    R* slist = reinterpret_cast<R*>(smem_raw);
+    __shared__ double red_a[kThreads / 32], red_b[kThreads / 32];
+
+    // H1 (device side): stage the value lists in shared memory, rounded to the evaluation type
+    if (p.stage_smem) {
+        for (uint32_t i = threadIdx.x; i < p.lists_total; i += kThreads) slist[i] = (R)p.lists[i];
+        __syncthreads();
+    }
+
+    const uint32_t lanes = SCHED == kSchedThread ? 1u : SCHED == kSchedWarp ? 32u : (uint32_t)kThreads;
+    const uint32_t lane = SCHED == kSchedThread ? 0u : SCHED == kSchedWarp ? (threadIdx.x & 31u) : threadIdx.x;
+    const uint64_t worker = SCHED == kSchedThread ? (uint64_t)blockIdx.x * kThreads + threadIdx.x
+                          : SCHED == kSchedWarp   ? ((uint64_t)blockIdx.x * kThreads + threadIdx.x) >> 5
+                                                  : (uint64_t)blockIdx.x;
+    uint64_t t = p.first + worker;
+    if (t >= p.end) return;                         // uniform per warp (WARP) / per CTA (CTA)
+
+    // H3: mixed-radix decode, once per worker with 64-bit arithmetic, then advanced by carries
+    uint32_t digit[ZMC_MAX_M];
+    if (p.end <= 0xFFFFFFFFull) {                   // whole range below 2^32: 32-bit division
+        uint32_t rest = (uint32_t)t;
+#pragma unroll
+        for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
+            if (i < M) {
+                const uint32_t q = rest / p.counts[i];
+                digit[i] = rest - q * p.counts[i];
+                rest = q;
+            } else {
+                digit[i] = 0;
+            }
+        }
+        digit[0] = rest;
+    } else {
+        uint64_t rest = t;
+#pragma unroll
+        for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
+            if (i < M) {
+                const uint64_t q = rest / p.counts[i];
+                digit[i] = (uint32_t)(rest - q * p.counts[i]);
+                rest = q;
+            } else {
+                digit[i] = 0;
+            }
+        }
+        digit[0] = (uint32_t)rest;
+    }
+
+    const uint32_t n = p.n;
+    const uint32_t n_full = n / S;                 // full groups; the last group may be clipped
+    const uint32_t rem = n - n_full * S;
+    const double inv_n = 1.0 / (double)n;
+
+    for (; t < p.end; t += p.stride) {
+        R x[ZMC_MAX_M];
+#pragma unroll
+        for (int i = 0; i < ZMC_MAX_M; ++i) {
+            if (i < M) {
+                const uint32_t idx = p.list_off[i] + digit[i];
+                x[i] = p.stage_smem ? slist[idx] : (R)__ldg(p.lists + idx);
+            } else {
+                x[i] = (R)0;
+            }
+        }
+        Fam fam;
+        fam.setup(x, p);
+        PhiloxPoint px;
+        px.init(t, p.rk);
+
+        uint32_t w[GS::NB * 4];
+        Accum<R> acc;
+        {   // shift K = g(sample 0): words 0..N-1
+            const int nb0 = (N + 3) >> 2;
+#pragma unroll
+            for (int b = 0; b < (kN ? (kN + 3) / 4 : ZMC_MAX_N / 4); ++b)
+                if (b < nb0) px.block((uint32_t)b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+            acc.K = fam.eval(w);
+        }
+
+        // H4 + H5 + H6: the hot loop
+        for (uint32_t g = lane; g < n_full; g += lanes) {
+            const uint32_t j0 = g * (uint32_t)NB;
+#pragma unroll
+            for (int b = 0; b < GS::NB; ++b)
+                if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+#pragma unroll
+            for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
+        }
+        if (rem != 0 && (n_full % lanes) == lane) {        // clipped last group: warp-uniform trip count
+            const uint32_t j0 = n_full * (uint32_t)NB;
+#pragma unroll
+            for (int b = 0; b < GS::NB; ++b)
+                if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+#pragma unroll
+            for (int s = 0; s < S - 1; ++s)
+                if ((uint32_t)s < rem) acc.add(fam.eval(&w[s * N]));
+        }
+
+        // H6: combine lanes (plain sums: the shift K is common to all lanes of the point)
+        double A = acc.A, B = acc.B;
+        if (SCHED != kSchedThread) {
+#pragma unroll
+            for (int m = 16; m >= 1; m >>= 1) {
+                A += __shfl_xor_sync(0xffffffffu, A, m);
+                B += __shfl_xor_sync(0xffffffffu, B, m);
+            }
+        }
+        if (SCHED == kSchedCta) {
+            const int warp = threadIdx.x >> 5;
+            if ((threadIdx.x & 31) == 0) { red_a[warp] = A; red_b[warp] = B; }
+            __syncthreads();
+            if (warp == 0) {
+                A = (threadIdx.x < kThreads / 32) ? red_a[threadIdx.x] : 0.0;
+                B = (threadIdx.x < kThreads / 32) ? red_b[threadIdx.x] : 0.0;
+#pragma unroll
+                for (int m = kThreads / 64; m >= 1; m >>= 1) {
+                    A += __shfl_xor_sync(0xffffffffu, A, m);
+                    B += __shfl_xor_sync(0xffffffffu, B, m);
+                }
+            }
+            __syncthreads();                       // red_* reused by the next point
+        }
+
+        // H7: finalise and store (coalesced across the warp in the THREAD schedule)
+        if (lane == 0) {
+            const double mean_g = (double)acc.K + A * inv_n;
+            double m2 = ::fma(-A * inv_n, A, B);
+            m2 = m2 > 0.0 ? m2 : 0.0;
+            const double mean = p.volume * mean_g;
+            const double serr = p.volume * sqrt(m2 / ((double)(n - 1) * (double)n));
+            const uint64_t o = t - p.out_base;
+            if (p.out_f32) {
+                static_cast<float*>(out_mean)[o] = (float)mean;
+                static_cast<float*>(out_stderr)[o] = (float)serr;
+            } else {
+                static_cast<double*>(out_mean)[o] = mean;
+                static_cast<double*>(out_stderr)[o] = serr;
+            }
+        }
+
+        // advance the digits by the worker stride (32-bit carries, no division)
+        uint32_t carry = 0;
+#pragma unroll
+        for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
+            if (i < M) {
+                uint32_t v = digit[i] + p.stride_digits[i] + carry;
+                carry = v >= p.counts[i] ? 1u : 0u;
+                digit[i] = v - (carry ? p.counts[i] : 0u);
+            }
+        }
+        digit[0] += p.stride_digits[0] + carry;
+    }
+}
+
+template <class Fam, int SCHED>
+cudaError_t launch_scan(const ScanParams& p, void* out_mean, void* out_stderr, int grid, size_t smem_bytes,
+                        cudaStream_t stream)
+{
+    auto kern = zmc_scan_kernel<Fam, SCHED>;
+    if (smem_bytes > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<grid, kThreads, smem_bytes, stream>>>(p, out_mean, out_stderr);
+    return cudaGetLastError();
+}
+
+// three table rows (one per schedule) for one family type; the type goes last because it contains commas
+#define ZMC_ENTRY(FAMILY_ID, NDIM, PREC, FAST, ...)                                                      \
+    {FAMILY_ID, NDIM, PREC, FAST, kSchedThread, &launch_scan<__VA_ARGS__, kSchedThread>,                \
+     (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedThread>},                                         \
+    {FAMILY_ID, NDIM, PREC, FAST, kSchedWarp, &launch_scan<__VA_ARGS__, kSchedWarp>,                    \
+     (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedWarp>},                                           \
+    {FAMILY_ID, NDIM, PREC, FAST, kSchedCta, &launch_scan<__VA_ARGS__, kSchedCta>,                      \
+     (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedCta>}
+
+// the three arithmetic variants of a family template F<R, ..., FAST>: fp64, fp32+MUFU, fp32 accurate
+#define ZMC_ENTRY_FIXED(FAMILY_ID, NDIM, F)                                  \
+    ZMC_ENTRY(FAMILY_ID, NDIM, ZMC_PREC_F64, 0, F<double, false>),           \
+    ZMC_ENTRY(FAMILY_ID, NDIM, ZMC_PREC_F32E, 1, F<float, true>),            \
+    ZMC_ENTRY(FAMILY_ID, NDIM, ZMC_PREC_F32E, 0, F<float, false>)
+#define ZMC_ENTRY_NDIM(FAMILY_ID, NDIM, F)                                   \
+    ZMC_ENTRY(FAMILY_ID, NDIM, ZMC_PREC_F64, 0, F<double, NDIM, false>),     \
+    ZMC_ENTRY(FAMILY_ID, NDIM, ZMC_PREC_F32E, 1, F<float, NDIM, true>),      \
+    ZMC_ENTRY(FAMILY_ID, NDIM, ZMC_PREC_F32E, 0, F<float, NDIM, false>)
+#define ZMC_ENTRY_DIAG(FAMILY_ID, F)                                         \
+    ZMC_ENTRY(FAMILY_ID, 0, ZMC_PREC_F64, 0, F<double>),                     \
+    ZMC_ENTRY(FAMILY_ID, 0, ZMC_PREC_F32E, 0, F<float>)
+
+}  // namespace zmc

@@ -1,0 +1,151 @@
+// zmc_math.cuh -- device arithmetic building blocks of the zmc_scan hot loop (sm_100a).
+//
+// H4 (sampler): Philox4x32-10 written from its definition (Salmon et al., SC'11; DESIGN.md
+// reading Q1/S2) with the per-point part of the first two rounds hoisted, and the exact uniforms
+// of reading S4 built by bit tricks (no I2F on the 16-lane XU pipe).
+// H5 (integrand): a branch-free fp64 sin(pi z) (exact range reduction in units of pi, degree-15
+// odd polynomial with immediate coefficients -- no table loads, no slow path) and thin wrappers
+// over the MUFU transcendentals for the fp32 path.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace zmc {
+
+// ------------------------------------------------------------------------------------------
+// Philox4x32-10.  Counter = (block j, 0, t lo, t hi), key = seed (stream layout S3).
+// rk[2r], rk[2r+1] are the round keys k0 + r*0x9E3779B9, k1 + r*0xBB67AE85 (host-computed,
+// read straight from the constant bank by LOP3).
+// With t fixed per grid point, counter words 2,3 and word 1 (= 0) are loop invariants, so round
+// 1 needs one multiply and round 2 one multiply: 18 IMAD.WIDE + 19 LOP3 per block instead of 20+20.
+// ------------------------------------------------------------------------------------------
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
+constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;
+
+struct PhiloxPoint {
+    uint32_t r1_c0, r1_c1;      // counter words 0,1 after round 1 (depend on t only)
+    uint32_t r1_x;              // t_hi ^ rk[1]: folded into word 2 of round 1
+    uint32_t r2_c3;             // counter word 3 after round 2 (t only)
+    uint32_t r2_e0, r2_e2;      // invariants folded into words 0 and 2 of round 2
+
+    __device__ __forceinline__ void init(uint64_t t, const uint32_t* __restrict__ rk) {
+        const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * t_lo;           // round 1, multiply of word 2
+        r1_c0 = (uint32_t)(p1 >> 32) ^ rk[0];                     // hi1 ^ c1(=0) ^ k0
+        r1_c1 = (uint32_t)p1;                                     // lo1
+        r1_x = t_hi ^ rk[1];
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * r1_c0;          // round 2, multiply of word 0
+        r2_c3 = (uint32_t)p0;                                     // lo0
+        r2_e2 = (uint32_t)(p0 >> 32) ^ rk[3];                     // hi0 ^ k1 (then ^ c3)
+        r2_e0 = r1_c1 ^ rk[2];                                    // c1 ^ k0 (then ^ hi1)
+    }
+
+    __device__ __forceinline__ void block(uint32_t j, const uint32_t* __restrict__ rk,
+                                          uint32_t (&out)[4]) const {
+        // round 1: only word 0 (= j) varies
+        uint64_t p0 = (uint64_t)kPhiloxM0 * j;
+        uint32_t c2 = (uint32_t)(p0 >> 32) ^ r1_x;
+        uint32_t c3 = (uint32_t)p0;
+        // round 2: word 0 is invariant
+        uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        uint32_t c0 = (uint32_t)(p1 >> 32) ^ r2_e0;
+        uint32_t c1 = (uint32_t)p1;
+        c2 = r2_e2 ^ c3;
+        c3 = r2_c3;
+#pragma unroll
+        for (int r = 2; r < 10; ++r) {
+            p0 = (uint64_t)kPhiloxM0 * c0;
+            p1 = (uint64_t)kPhiloxM1 * c2;
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
+            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
+            c1 = (uint32_t)p1;
+            c3 = (uint32_t)p0;
+            c0 = n0;
+            c2 = n2;
+        }
+        out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// Uniforms (reading S4).  unit(w) is f = 1 + (w >> drop)*2^-mant in [1,2), built with one
+// funnel shift (fp32) or a funnel shift and a shift (fp64); u = f - (1 - eps) is then the exact
+// lattice value (2(w>>9)+1)*2^-24 resp. (2w+1)*2^-33.  Families fold the "- (1 - eps)" into
+// per-point constants, so the hot loop spends one FMA per dimension.
+// ------------------------------------------------------------------------------------------
+template <typename R> struct Real;
+
+template <> struct Real<float> {
+    static __device__ __forceinline__ float unit(uint32_t w) {
+        return __uint_as_float(__funnelshift_r(w, 0x7Fu, 9));        // (w>>9) | 0x3F800000
+    }
+    static __device__ __forceinline__ float one_minus_eps() { return 0x1.fffffep-1f; }   // 1 - 2^-24
+    static __device__ __forceinline__ float fma(float a, float b, float c) { return fmaf(a, b, c); }
+};
+
+template <> struct Real<double> {
+    static __device__ __forceinline__ double unit(uint32_t w) {
+        return __hiloint2double((int)__funnelshift_r(w, 0x3FFu, 12), (int)(w << 20));   // 1 + w*2^-32
+    }
+    static __device__ __forceinline__ double one_minus_eps() { return 0x1.fffffffcp-1; }  // 1 - 2^-33
+    static __device__ __forceinline__ double fma(double a, double b, double c) { return ::fma(a, b, c); }
+};
+
+// exact lattice uniform u in (0,1)
+template <typename R> __device__ __forceinline__ R uniform(uint32_t w) {
+    return Real<R>::unit(w) - Real<R>::one_minus_eps();
+}
+
+// ------------------------------------------------------------------------------------------
+// fp64 sin(pi z), any |z| < 2^51.  k = rint(z) by the magic-number add, r = z - k exact,
+// sin(pi z) = (-1)^k sin(pi r), |r| <= 1/2; odd polynomial r*P7(r^2), max error 2.4e-16
+// (Chebyshev-node fit of sin(pi sqrt(s))/sqrt(s) on [0,1/4]).  13 fp64-pipe ops + 2 ALU ops.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double sinpi_f64(double z) {
+    const double kMagic = 6755399441055744.0;                  // 1.5 * 2^52
+    const double kf = z + kMagic;
+    const double r = z - (kf - kMagic);
+    const double s = r * r;
+    double p = -0x1.62903d02bb153p-16;
+    p = ::fma(p, s, 0x1.e89f6fe44fe7bp-12);
+    p = ::fma(p, s, -0x1.e30631bdf732dp-8);
+    p = ::fma(p, s, 0x1.5078327046959p-4);
+    p = ::fma(p, s, -0x1.32d2cce1ea145p-1);
+    p = ::fma(p, s, 0x1.466bc677522bdp+1);
+    p = ::fma(p, s, -0x1.4abbce625bd83p+2);
+    const double rs = r * s;
+    const double v = ::fma(rs, p, r * 0x1.921fb54442d17p+1) ;
+    // sign flip for odd k: xor bit 0 of k into the sign bit
+    const int hi = __double2hiint(v) ^ (__double2loint(kf) << 31);
+    return __hiloint2double(hi, __double2loint(v));
+}
+
+// Transcendentals of the evaluation type.  FAST selects the MUFU forms for fp32 (reading:
+// north_star "fast-math transcendentals only where the tolerance allows"); fp64 ignores it.
+template <typename R, bool FAST> struct Fn;
+
+template <bool FAST> struct Fn<double, FAST> {
+    // arguments are phases in units of pi ("turns/2"): families pre-scale their coefficients by 1/pi
+    static __device__ __forceinline__ double sin_pi(double z) { return sinpi_f64(z); }
+    static __device__ __forceinline__ double exp2_neg(double e) { return ::exp2(-e); }
+    static constexpr bool kPhaseInPi = true;
+};
+
+template <> struct Fn<float, true> {
+    // phase in radians: sin.approx = FMUL(1/2pi) + MUFU.SIN
+    static __device__ __forceinline__ float sin_rad(float a) { return __sinf(a); }
+    static __device__ __forceinline__ float cos_rad(float a) { return __cosf(a); }
+    static __device__ __forceinline__ float exp2_neg(float e) {            // 2^-e: one MUFU.EX2
+        float r;
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-e));
+        return r;
+    }
+};
+
+template <> struct Fn<float, false> {
+    static __device__ __forceinline__ float sin_rad(float a) { return sinf(a); }
+    static __device__ __forceinline__ float cos_rad(float a) { return cosf(a); }
+    static __device__ __forceinline__ float exp2_neg(float e) { return exp2f(-e); }
+};
+
+}  // namespace zmc

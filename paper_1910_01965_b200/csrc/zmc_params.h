@@ -1,0 +1,42 @@
+// zmc_params.h -- the kernel argument block (host fills it, kernels read it from the constant bank).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/zmc.h"
+
+namespace zmc {
+
+struct ScanParams {
+    uint64_t first, end;          // flat indices [first, end) of this launch (GLOBAL indices, reading S3)
+    uint64_t out_base;            // element written = t - out_base
+    uint64_t stride;              // points between two consecutive points of one worker
+    const double* lists;          // device: the M value lists, concatenated
+    uint32_t rk[20];              // Philox round keys: rk[2r] = k0 + r*W0, rk[2r+1] = k1 + r*W1
+    uint32_t n;                   // samples per point
+    uint32_t n_dim, n_par;        // N, M
+    uint32_t lists_total;         // total list entries
+    uint32_t stage_smem;          // 1: lists are staged in shared memory (else read through L1/L2)
+    uint32_t out_f32;             // 1: outputs are float
+    uint32_t counts[ZMC_MAX_M];   // list lengths L_i
+    uint32_t list_off[ZMC_MAX_M]; // offset of list i in `lists`
+    uint32_t stride_digits[ZMC_MAX_M];  // mixed-radix digits of `stride` (top digit unbounded)
+    double a[ZMC_MAX_N], width[ZMC_MAX_N];   // box; in F32E mode already rounded to float (mirror, reading S5)
+    double volume;                // prod_k width_k, k ascending
+    double consts[ZMC_MAX_CONSTS];
+};
+
+enum { kSchedThread = ZMC_SCHED_THREAD, kSchedWarp = ZMC_SCHED_WARP, kSchedCta = ZMC_SCHED_CTA };
+
+constexpr int kThreads = 256;      // CTA size of every schedule
+
+// launcher signature shared by the dispatch table (zmc_api.cu) and the instantiation units
+typedef cudaError_t (*LaunchFn)(const ScanParams& p, void* out_mean, void* out_stderr, int grid,
+                                size_t smem_bytes, cudaStream_t stream);
+
+struct KernelEntry {
+    int family, n_dim /* 0 = any (runtime N) */, precision, fast, schedule;
+    LaunchFn launch;
+    const void* func;              // for occupancy queries / attributes
+};
+
+}  // namespace zmc

@@ -1,0 +1,123 @@
+"""CPU-only checks of the C-ABI boundary: the library loads, exports every symbol include/zmc.h
+declares, and its pure-host entry points (validation, schedule choice, batch cutting) behave.
+No compute call is made here (there is no GPU and no CPU fallback)."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1910_01965_b200 import binding as zb
+from paper_1910_01965_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = zb.load()
+    header = open(os.path.join(ROOT, "include", "zmc.h")).read()
+    declared = set(re.findall(r"ZMC_API[^;(]*?\b(zmc_\w+)\s*\(", header))
+    assert declared == set(zb.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert "sm_100a" in zb.zmc_version()
+
+
+def test_struct_layouts_match_header_sizes(tmp_path):
+    # the header is plain C99: compile it with gcc and compare struct sizes with the ctypes mirrors
+    import ctypes
+    import subprocess
+    src = tmp_path / "sz.c"
+    src.write_text('#include <stdio.h>\n#include "zmc.h"\nint main(void){printf("%zu %zu %zu %zu\\n",'
+                   'sizeof(zmc_options),sizeof(zmc_timing),sizeof(zmc_param_list),sizeof(zmc_integrand_info));return 0;}\n')
+    exe = tmp_path / "sz"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)],
+                   check=True)
+    sizes = [int(v) for v in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
+    assert sizes == [ctypes.sizeof(zb.zmc_options), ctypes.sizeof(zb.zmc_timing), ctypes.sizeof(zb.zmc_param_list),
+                     ctypes.sizeof(zb.zmc_integrand_info)]
+
+
+def test_integrand_table():
+    fams = {f["id"]: f for f in zb.zmc_integrands()}
+    assert set(fams) == {1, 2, 3, 4, 5, 6, 100, 101, 102, 103}
+    assert fams[3]["n_consts"] == 1 and fams[3]["M"] == (3, 3)
+    assert fams[4]["N"] == (6, 6) and fams[5]["M"] == (5, 5)
+
+
+def test_every_config_validates_with_expected_grid_size():
+    sizes = {1: 10 ** 3, 2: 10 ** 6, 3: 8 * 10 ** 6, 4: 10 ** 8, 5: 10 ** 10}
+    for k, G in sizes.items():
+        w = wl.config(k)
+        st, g = zb.zmc_validate(w.integrand_id, w.bounds, w.lists, w.n_samples, precision=w.precision,
+                                consts=w.consts)
+        assert (st, g) == (zb.ZMC_OK, G) and w.G == G
+
+
+def test_validation_errors():
+    w = wl.config(1, scale=[4], n_samples=10)
+    ok = dict(integrand_id=1, bounds=w.bounds, lists=w.lists, n_samples=10)
+
+    def st(**kw):
+        a = dict(ok)
+        a.update(kw)
+        extra = {k: a.pop(k) for k in list(a) if k not in ("integrand_id", "bounds", "lists", "n_samples")}
+        return zb.zmc_validate(a["integrand_id"], a["bounds"], a["lists"], a["n_samples"], **extra)[0]
+
+    assert st() == zb.ZMC_OK
+    assert st(n_samples=1) == zb.ZMC_ERR_INVALID_ARG
+    assert st(n_samples=1 << 32) == zb.ZMC_ERR_INVALID_ARG
+    assert st(bounds=[0.0, 0.0]) == zb.ZMC_ERR_INVALID_ARG
+    assert st(bounds=[0.0, float("inf")]) == zb.ZMC_ERR_INVALID_ARG
+    assert st(lists=[np.array([1.0, float("nan")])]) == zb.ZMC_ERR_INVALID_ARG
+    assert st(integrand_id=42) == zb.ZMC_ERR_UNKNOWN_INTEGRAND
+    assert st(integrand_id=2) == zb.ZMC_ERR_SHAPE_MISMATCH
+    assert st(integrand_id=3, lists=[w.lists[0]] * 3) == zb.ZMC_ERR_SHAPE_MISMATCH      # c3 needs consts={u}
+    assert st(integrand_id=3, lists=[w.lists[0]] * 3, consts=[0.25]) == zb.ZMC_OK
+    assert st(integrand_id=101, consts=[1.0]) == zb.ZMC_ERR_SHAPE_MISMATCH                # echo index >= M
+    assert st(first_index=5) == zb.ZMC_ERR_INVALID_ARG
+    assert st(first_index=2, count=3) == zb.ZMC_ERR_INVALID_ARG
+    assert st(first_index=2, count=2) == zb.ZMC_OK
+    assert st(precision=7) == zb.ZMC_ERR_INVALID_ARG
+    assert st(schedule=9) == zb.ZMC_ERR_INVALID_ARG
+    big = [np.zeros(1 << 17)] * 3                                                         # 2^51 points
+    assert st(integrand_id=6, lists=big) == zb.ZMC_ERR_GRID_TOO_LARGE
+    assert st(integrand_id=6, bounds=[0.0, 1.0] * 16, n_samples=(1 << 30) + 1) == zb.ZMC_ERR_INVALID_ARG
+    assert "invalid" in zb.zmc_status_string(zb.ZMC_ERR_INVALID_ARG)
+
+
+def test_schedule_choice_follows_design_table():
+    # cfg1 CTA, cfg2 WARP, cfg3-5 THREAD
+    expect = {1: zb.ZMC_SCHED_CTA, 2: zb.ZMC_SCHED_WARP, 3: zb.ZMC_SCHED_THREAD, 4: zb.ZMC_SCHED_THREAD}
+    for k, s in expect.items():
+        w = wl.config(k)
+        assert zb.zmc_pick_schedule(w.G, w.n_samples, w.N) == s
+    w = wl.config(5)
+    assert zb.zmc_pick_schedule(1 << 28, w.n_samples, w.N) == zb.ZMC_SCHED_THREAD
+    assert zb.zmc_pick_schedule(10, 8, 1) == zb.ZMC_SCHED_THREAD          # too few samples to split
+
+
+@pytest.mark.parametrize("first,count,bp", [(0, 10 ** 10, 1 << 28), (5, 1000, 97), (0, 7, 0), (3, 7, 100), (0, 8, 4)])
+def test_batch_cutting_covers_range_exactly(first, count, bp):
+    nb, _, _ = zb.zmc_batch_range(first, count, bp, 0)
+    pos = first
+    for b in range(nb):
+        n2, f, c = zb.zmc_batch_range(first, count, bp, b)
+        assert n2 == nb and f == pos and c >= 1
+        assert c == (bp if bp and b < nb - 1 else c)
+        pos += c
+    assert pos == first + count
+    if (first, count, bp) == (0, 10 ** 10, 1 << 28):
+        assert nb == 38 and zb.zmc_batch_range(first, count, bp, 37)[2] == 67_888_128
+
+
+def test_compute_call_fails_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    w = wl.config(1, scale=[4], n_samples=10)
+    mean, err = np.zeros(4), np.zeros(4)
+    with pytest.raises(zb.ZmcError) as ei:
+        zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, mean, err, stream=0)
+    assert ei.value.status == zb.ZMC_ERR_CUDA
+    assert np.all(mean == 0) and np.all(err == 0)

@@ -1,0 +1,187 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star, reading Q12 in DESIGN.md):
+  fp64 path : |d mean| <= 1e-10 * max(|mean_o|, stderr_o),  |d stderr| <= 1e-10 * stderr_o
+  F32E path : |d| <= 1e-4 * |oracle| + 1e-6   (mean and stderr)
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import zmc_oracle as orc
+from paper_1910_01965_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+NT = min(16, os.cpu_count() or 1)
+SCHEDS = {"thread": 1, "warp": 2, "cta": 3}
+
+
+def _zb():
+    from paper_1910_01965_b200 import binding
+    return binding
+
+
+def assert_parity(w, mean, err, mean_o, err_o):
+    mean, err = np.asarray(mean, dtype=np.float64), np.asarray(err, dtype=np.float64)
+    if w.precision == wl.PREC_F64 and not w.out_f32:
+        tol_m = 1e-10 * np.maximum(np.abs(mean_o), err_o)
+        tol_e = 1e-10 * err_o
+        bad_m = np.abs(mean - mean_o) > tol_m + 1e-300
+        bad_e = np.abs(err - err_o) > tol_e + 1e-300
+    else:
+        bad_m = np.abs(mean - mean_o) > 1e-4 * np.abs(mean_o) + 1e-6
+        bad_e = np.abs(err - err_o) > 1e-4 * np.abs(err_o) + 1e-6
+    assert not bad_m.any(), f"mean: {bad_m.sum()} of {len(mean)} off, worst {np.abs(mean - mean_o).max()}"
+    assert not bad_e.any(), f"stderr: {bad_e.sum()} of {len(err)} off, worst {np.abs(err - err_o).max()}"
+
+
+def run_gpu(w, **kw):
+    import torch
+    zb = _zb()
+    m, e, _ = zb.scan_workload(w, **kw)
+    torch.cuda.synchronize()
+    return m.cpu().numpy(), e.cpu().numpy()
+
+
+REDUCED = {
+    "cfg1": lambda: wl.config(1, scale=[257]),
+    "cfg1_n_ragged": lambda: wl.config(1, scale=[33], n_samples=10_007),
+    "cfg2": lambda: wl.config(2, scale=[37, 41], n_samples=3001),
+    "cfg3": lambda: wl.config(3, scale=[13, 11, 17]),
+    "cfg3_N5": lambda: _c3_n(5),
+    "cfg3_N9_runtime": lambda: _c3_n(9),
+    "cfg4": lambda: wl.config(4, scale=[9, 7, 5, 11], n_samples=1001),
+    "cfg5": lambda: wl.config(5, scale=[5, 4, 3, 6, 7], n_samples=259),
+    "eq2_M2_N3": lambda: wl.paper_eq2(2, 3, n_samples=2000, L=31),
+    "eq2_M4_N4_f32": lambda: wl.paper_eq2(4, 4, n_samples=500, L=7, precision=wl.PREC_F32E),
+    "eq4": lambda: wl.paper_eq4(n_samples=3000, L=6),
+    "eq4_f32": lambda: wl.paper_eq4(n_samples=3000, L=6, precision=wl.PREC_F32E),
+}
+
+
+def _c3_n(N):
+    w = wl.config(3, scale=[7, 5, 6], n_samples=1501)
+    w.bounds = np.array([0.0, 1.0] * N)
+    return w
+
+
+@pytest.mark.parametrize("name", sorted(REDUCED))
+@pytest.mark.parametrize("sched", sorted(SCHEDS))
+def test_parity_reduced(name, sched):
+    w = REDUCED[name]()
+    w.host_out, w.batch_points = False, 0
+    rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
+    assert rc == 0
+    mean, err = run_gpu(w, schedule=SCHEDS[sched])
+    assert_parity(w, mean, err, mean_o, err_o)
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5", "eq4_f32"])
+def test_parity_f32_accurate_math(name):
+    w = REDUCED[name]()
+    w.host_out, w.batch_points = False, 0
+    rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
+    mean, err = run_gpu(w, fast_math=0)
+    assert_parity(w, mean, err, mean_o, err_o)
+
+
+@pytest.mark.parametrize("prec", [wl.PREC_F64, wl.PREC_F32E])
+@pytest.mark.parametrize("fid,consts", [(wl.D_CONST_ONE, []), (wl.D_PARAM_ECHO, [2.0]), (wl.D_LIN_Y, [1.0]),
+                                        (wl.D_POLY, [])])
+def test_diagnostic_families(fid, consts, prec):
+    w = wl.Workload("diag", fid, np.array([0.0, 2.0, -1.0, 0.5, 3.0, 3.25]),
+                    [np.arange(4.0) + 0.25, np.arange(3.0) * 1.5, np.array([7.0, 9.0, 11.0, 13.0, 15.0])],
+                    37, 5, prec, np.array(consts))
+    rc, mean_o, err_o = orc.scan_workload(w)
+    assert rc == 0
+    for sched in (1, 2, 3):
+        mean, err = run_gpu(w, schedule=sched)
+        if fid in (wl.D_CONST_ONE, wl.D_PARAM_ECHO):
+            assert np.array_equal(mean, mean_o)          # decode + volume: bit-exact
+            assert np.all(err == 0.0)
+        else:
+            assert_parity(w, mean, err, mean_o, err_o)
+
+
+def test_batch_and_subrange_invariance_bit_exact():
+    import torch
+    zb = _zb()
+    w = wl.config(5, scale=[5, 4, 3, 6, 7], n_samples=64)
+    w.host_out = False
+    for sched in (1, 2, 3):
+        full_m, full_e = run_gpu(w, schedule=sched, batch_points=0)
+        for bp in (1, 97, 1000):
+            m, e = run_gpu(w, schedule=sched, batch_points=bp)
+            assert np.array_equal(m, full_m) and np.array_equal(e, full_e)
+        m, e = run_gpu(w, schedule=sched, first_index=1234, count=777, batch_points=100)
+        assert np.array_equal(m, full_m[1234:1234 + 777]) and np.array_equal(e, full_e[1234:1234 + 777])
+        # host output through the staging double-buffer
+        hm, he, _ = zb.scan_workload(w, schedule=sched, batch_points=500, host_out=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(hm.numpy(), full_m) and np.array_equal(he.numpy(), full_e)
+
+
+def test_indices_above_2_pow_32():
+    # decode and Philox counter must be 64-bit clean: sub-ranges straddling 2^32 and 2^33
+    counts = (70000, 70000, 3)
+    lists = [wl.linspace(0.5, 5.0, counts[0]), wl.linspace(0.5, 5.0, counts[1]), np.array([1.0, 2.0, 3.0])]
+    w = wl.Workload("big", wl.P6_SIN_SUM, np.array([0.0, 1.0, 0.0, 2.0]), lists, 200, 9, wl.PREC_F64, np.zeros(0))
+    for first in ((1 << 32) - 300, (1 << 33) - 5, w.G - 600):
+        count = 600
+        rc, mean_o, err_o = orc.scan_workload(w, first, count, n_threads=NT)
+        assert rc == 0
+        for sched in (1, 2, 3):
+            mean, err = run_gpu(w, schedule=sched, first_index=first, count=count, batch_points=256)
+            assert_parity(w, mean, err, mean_o, err_o)
+
+
+def test_nearly_constant_integrand_stderr():
+    # hard part 3 of SURVEY.md section 7: raw sums lose the stderr of a nearly constant integrand
+    w = wl.config(1, scale=[5], n_samples=10_000)
+    w.lists = [np.array([1e-4, 3e-4, 1e-3, 0.01, 0.1])]
+    rc, mean_o, err_o = orc.scan_workload(w)
+    for sched in (1, 2, 3):
+        mean, err = run_gpu(w, schedule=sched)
+        assert_parity(w, mean, err, mean_o, err_o)
+
+
+def test_stream_ordering_and_default_entry_point():
+    import torch
+    zb = _zb()
+    w = wl.config(2, scale=[20, 30], n_samples=500)
+    rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
+    st = torch.cuda.Stream()
+    mean = torch.zeros(w.G, dtype=torch.float64, device="cuda")
+    err = torch.zeros(w.G, dtype=torch.float64, device="cuda")
+    st.wait_stream(torch.cuda.current_stream())
+    zb.zmc_scan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, mean, err, stream=st)
+    st.synchronize()
+    assert_parity(w, mean.cpu().numpy(), err.cpu().numpy(), mean_o, err_o)
+
+
+def test_errors_leave_outputs_untouched():
+    import torch
+    zb = _zb()
+    w = wl.config(1, scale=[8], n_samples=10)
+    mean = torch.full((8,), -7.0, dtype=torch.float64, device="cuda")
+    err = torch.full((8,), -7.0, dtype=torch.float64, device="cuda")
+    for bad in ({"n_samples": 1}, {"integrand_id": 99}, {"bounds": [1.0, 0.0]}):
+        args = dict(integrand_id=w.integrand_id, bounds=w.bounds, lists=w.lists, n_samples=w.n_samples, seed=1)
+        args.update(bad)
+        with pytest.raises(zb.ZmcError):
+            zb.zmc_scan_ex(args["integrand_id"], args["bounds"], args["lists"], args["n_samples"], args["seed"],
+                           mean, err)
+    torch.cuda.synchronize()
+    assert torch.all(mean == -7.0) and torch.all(err == -7.0)
+
+
+def test_timing_struct():
+    zb = _zb()
+    w = wl.config(5, scale=[6, 6, 6, 6, 6], n_samples=64)
+    w.batch_points = 2000
+    m, e, tm = zb.scan_workload(w, timing=True)
+    assert tm["n_batches"] == 4 and tm["gpu_launches"] == 4
+    assert tm["d2h_bytes"] == 2 * 4 * w.G and tm["h2d_bytes"] == 8 * 30
+    assert tm["kernel_ms"] > 0 and tm["wall_ms"] >= tm["kernel_ms"] * 0.99 and tm["d2h_ms"] > 0
