@@ -87,7 +87,7 @@ template <> struct Real<double> {
     static __device__ __forceinline__ double unit(uint32_t w) {
         return __hiloint2double((int)__funnelshift_r(w, 0x3FFu, 12), (int)(w << 20));   // 1 + w*2^-32
     }
-    static __device__ __forceinline__ double one_minus_eps() { return 0x1.fffffffcp-1; }  // 1 - 2^-33
+    static __device__ __forceinline__ double one_minus_eps() { return 0x1.ffffffffp-1; }   // 1 - 2^-33
     static __device__ __forceinline__ double fma(double a, double b, double c) { return ::fma(a, b, c); }
 };
 
