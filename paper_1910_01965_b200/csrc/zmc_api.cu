@@ -408,10 +408,11 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
         if (n_batches > 1 && !s->stage[1]) ZMC_CUDA(cudaMalloc(&s->stage[1], s->stage_cap));
     }
 
-    int occ = 0;
-    ZMC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern->func, kThreads, smem_bytes));
-    if (occ < 1) occ = 1;
-    const uint64_t max_grid = (uint64_t)occ * (uint64_t)s->sm_count;
+    // One worker (thread / warp / CTA) per grid point, one CTA per `per_cta` points: the hardware CTA scheduler
+    // balances the load.  A batch larger than kMaxLaunchPoints is cut into several launches so that local point
+    // indices and the grid size stay 32-bit.
+    const uint64_t per_cta = schedule == ZMC_SCHED_THREAD ? kThreads : schedule == ZMC_SCHED_WARP ? kThreads / 32 : 1;
+    constexpr uint64_t kMaxLaunchPoints = 1ull << 30;
 
     std::vector<TimedSpan> t_kernel, t_copy;
     int64_t launches = 0;
@@ -419,33 +420,35 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
     for (int64_t b = 0; b < n_batches; ++b) {
         uint64_t bf = 0, bc = 0;
         zmc_batch_range(first, count, o.batch_points, b, &bf, &bc);
-        const uint64_t per_cta = schedule == ZMC_SCHED_THREAD ? kThreads : schedule == ZMC_SCHED_WARP ? kThreads / 32 : 1;
-        uint64_t grid = (bc + per_cta - 1) / per_cta;
-        if (grid > max_grid) grid = max_grid;
-        p.first = bf;
-        p.end = bf + bc;
-        p.stride = grid * per_cta;
-        {   // mixed-radix digits of the stride (top digit unbounded)
-            uint64_t rest = p.stride;
-            for (int i = M - 1; i >= 1; --i) { p.stride_digits[i] = (uint32_t)(rest % p.counts[i]); rest /= p.counts[i]; }
-            p.stride_digits[0] = (uint32_t)(rest > 0xFFFFFFFFull ? 0xFFFFFFFFull : rest);
-        }
         void *dst_mean, *dst_err;
+        uint64_t out_base;                     // flat index of element 0 of dst_mean / dst_err
         const int buf = (int)(b & 1);
         if (host_out) {
             if (s->stage_used[buf]) ZMC_CUDA(cudaStreamWaitEvent(stream, s->stage_free[buf], 0));
             dst_mean = s->stage[buf];
             dst_err = static_cast<char*>(s->stage[buf]) + (size_t)batch_max * elem_out;
-            p.out_base = bf;
+            out_base = bf;
         } else {
             dst_mean = out_mean;
             dst_err = out_stderr;
-            p.out_base = first;
+            out_base = first;
         }
         TimedSpan tk;
         if (timing) { ZMC_CUDA(new_tev(&tk.a)); ZMC_CUDA(new_tev(&tk.b)); ZMC_CUDA(cudaEventRecord(tk.a, stream)); }
-        ZMC_CUDA(kern->launch(p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
-        ++launches;
+        for (uint64_t lf = bf; lf < bf + bc; lf += kMaxLaunchPoints) {
+            const uint64_t lc = (bf + bc - lf < kMaxLaunchPoints) ? bf + bc - lf : kMaxLaunchPoints;
+            p.first = lf;
+            p.count = (uint32_t)lc;
+            p.out_off = lf - out_base;
+            {   // H3, 64-bit part: mixed-radix digits of the launch's first flat index
+                uint64_t rest = lf;
+                for (int i = M - 1; i >= 1; --i) { p.base_digits[i] = (uint32_t)(rest % p.counts[i]); rest /= p.counts[i]; }
+                p.base_digits[0] = (uint32_t)rest;
+            }
+            const uint64_t grid = (lc + per_cta - 1) / per_cta;
+            ZMC_CUDA(kern->launch(p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
+            ++launches;
+        }
         if (timing) { ZMC_CUDA(cudaEventRecord(tk.b, stream)); t_kernel.push_back(tk); }
 
         if (host_out) {   // H8: copy batch b on the side stream while batch b+1 computes

@@ -64,42 +64,38 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
         __syncthreads();
     }
 
+    // One grid point per worker (thread / warp / CTA); the grid has one CTA per kThreads / 8 / 1 points, so the
+    // hardware CTA scheduler balances the load and refills every slot a finished CTA frees.
     const uint32_t lanes = SCHED == kSchedThread ? 1u : SCHED == kSchedWarp ? 32u : (uint32_t)kThreads;
     const uint32_t lane = SCHED == kSchedThread ? 0u : SCHED == kSchedWarp ? (threadIdx.x & 31u) : threadIdx.x;
-    const uint64_t worker = SCHED == kSchedThread ? (uint64_t)blockIdx.x * kThreads + threadIdx.x
-                          : SCHED == kSchedWarp   ? ((uint64_t)blockIdx.x * kThreads + threadIdx.x) >> 5
-                                                  : (uint64_t)blockIdx.x;
-    uint64_t t = p.first + worker;
-    if (t >= p.end) return;                         // uniform per warp (WARP) / per CTA (CTA)
+    const uint32_t local = SCHED == kSchedThread ? blockIdx.x * kThreads + threadIdx.x
+                         : SCHED == kSchedWarp   ? blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5)
+                                                 : blockIdx.x;
+    if (local >= p.count) return;                   // uniform per warp (WARP) / per CTA (CTA)
+    const uint64_t t = p.first + local;
 
-    // H3: mixed-radix decode, once per worker with 64-bit arithmetic, then advanced by carries
-    uint32_t digit[ZMC_MAX_M];
-    if (p.end <= 0xFFFFFFFFull) {                   // whole range below 2^32: 32-bit division
-        uint32_t rest = (uint32_t)t;
+    // H3: mixed-radix decode.  digits(t) = digits(first) + digits(local) with carries: the 64-bit part was done on
+    // the host, the per-point part is 32-bit division only.
+    R x[ZMC_MAX_M];
+    {
+        uint32_t rest = local, carry = 0;
 #pragma unroll
         for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
             if (i < M) {
-                const uint32_t q = rest / p.counts[i];
-                digit[i] = rest - q * p.counts[i];
+                const uint32_t L = p.counts[i];
+                const uint32_t q = rest / L;
+                uint32_t d = p.base_digits[i] + (rest - q * L) + carry;
+                carry = d >= L ? 1u : 0u;
+                d -= carry ? L : 0u;
                 rest = q;
+                const uint32_t idx = p.list_off[i] + d;
+                x[i] = p.stage_smem ? slist[idx] : (R)__ldg(p.lists + idx);
             } else {
-                digit[i] = 0;
+                x[i] = (R)0;
             }
         }
-        digit[0] = rest;
-    } else {
-        uint64_t rest = t;
-#pragma unroll
-        for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
-            if (i < M) {
-                const uint64_t q = rest / p.counts[i];
-                digit[i] = (uint32_t)(rest - q * p.counts[i]);
-                rest = q;
-            } else {
-                digit[i] = 0;
-            }
-        }
-        digit[0] = (uint32_t)rest;
+        const uint32_t idx0 = p.list_off[0] + p.base_digits[0] + rest + carry;
+        x[0] = p.stage_smem ? slist[idx0] : (R)__ldg(p.lists + idx0);
     }
 
     const uint32_t n = p.n;
@@ -107,104 +103,83 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     const uint32_t rem = n - n_full * S;
     const double inv_n = 1.0 / (double)n;
 
-    for (; t < p.end; t += p.stride) {
-        R x[ZMC_MAX_M];
-#pragma unroll
-        for (int i = 0; i < ZMC_MAX_M; ++i) {
-            if (i < M) {
-                const uint32_t idx = p.list_off[i] + digit[i];
-                x[i] = p.stage_smem ? slist[idx] : (R)__ldg(p.lists + idx);
-            } else {
-                x[i] = (R)0;
-            }
-        }
-        Fam fam;
-        fam.setup(x, p);
-        PhiloxPoint px;
-        px.init(t, p.rk);
+    Fam fam;
+    fam.setup(x, p);
+    PhiloxPoint px;
+    px.init(t, p.rk);
 
-        uint32_t w[GS::NB * 4];
-        Accum<R> acc;
-        {   // shift K = g(sample 0): words 0..N-1
-            const int nb0 = (N + 3) >> 2;
+    uint32_t w[GS::NB * 4];
+    Accum<R> acc;
+    {   // shift K = g(sample 0): words 0..N-1
+        const int nb0 = (N + 3) >> 2;
 #pragma unroll
-            for (int b = 0; b < (kN ? (kN + 3) / 4 : ZMC_MAX_N / 4); ++b)
-                if (b < nb0) px.block((uint32_t)b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
-            acc.K = fam.eval(w);
-        }
+        for (int b = 0; b < (kN ? (kN + 3) / 4 : ZMC_MAX_N / 4); ++b)
+            if (b < nb0) px.block((uint32_t)b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+        acc.K = fam.eval(w);
+    }
 
-        // H4 + H5 + H6: the hot loop
-        for (uint32_t g = lane; g < n_full; g += lanes) {
-            const uint32_t j0 = g * (uint32_t)NB;
+    // H4 + H5 + H6: the hot loop
+    for (uint32_t g = lane; g < n_full; g += lanes) {
+        const uint32_t j0 = g * (uint32_t)NB;
+        if constexpr (kN != 0) {
+            px.template blocks<GS::NB>(j0, p.rk, w);
+        } else {
 #pragma unroll
             for (int b = 0; b < GS::NB; ++b)
                 if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
-#pragma unroll
-            for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
         }
-        if (rem != 0 && (n_full % lanes) == lane) {        // clipped last group: warp-uniform trip count
-            const uint32_t j0 = n_full * (uint32_t)NB;
 #pragma unroll
-            for (int b = 0; b < GS::NB; ++b)
-                if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+        for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
+    }
+    if (rem != 0 && (n_full % lanes) == lane) {        // clipped last group: warp-uniform trip count
+        const uint32_t j0 = n_full * (uint32_t)NB;
 #pragma unroll
-            for (int s = 0; s < S - 1; ++s)
-                if ((uint32_t)s < rem) acc.add(fam.eval(&w[s * N]));
-        }
+        for (int b = 0; b < GS::NB; ++b)
+            if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+#pragma unroll
+        for (int s = 0; s < S - 1; ++s)
+            if ((uint32_t)s < rem) acc.add(fam.eval(&w[s * N]));
+    }
 
-        // H6: combine lanes (plain sums: the shift K is common to all lanes of the point)
-        double A = acc.A, B = acc.B;
-        if (SCHED != kSchedThread) {
+    // H6: combine lanes (plain sums: the shift K is common to all lanes of the point)
+    double A = acc.A, B = acc.B;
+    if (SCHED != kSchedThread) {
 #pragma unroll
-            for (int m = 16; m >= 1; m >>= 1) {
+        for (int m = 16; m >= 1; m >>= 1) {
+            A += __shfl_xor_sync(0xffffffffu, A, m);
+            B += __shfl_xor_sync(0xffffffffu, B, m);
+        }
+    }
+    if (SCHED == kSchedCta) {
+        const int warp = threadIdx.x >> 5;
+        if ((threadIdx.x & 31) == 0) { red_a[warp] = A; red_b[warp] = B; }
+        __syncthreads();
+        if (warp == 0) {
+            A = (threadIdx.x < kThreads / 32) ? red_a[threadIdx.x] : 0.0;
+            B = (threadIdx.x < kThreads / 32) ? red_b[threadIdx.x] : 0.0;
+#pragma unroll
+            for (int m = kThreads / 64; m >= 1; m >>= 1) {
                 A += __shfl_xor_sync(0xffffffffu, A, m);
                 B += __shfl_xor_sync(0xffffffffu, B, m);
             }
         }
-        if (SCHED == kSchedCta) {
-            const int warp = threadIdx.x >> 5;
-            if ((threadIdx.x & 31) == 0) { red_a[warp] = A; red_b[warp] = B; }
-            __syncthreads();
-            if (warp == 0) {
-                A = (threadIdx.x < kThreads / 32) ? red_a[threadIdx.x] : 0.0;
-                B = (threadIdx.x < kThreads / 32) ? red_b[threadIdx.x] : 0.0;
-#pragma unroll
-                for (int m = kThreads / 64; m >= 1; m >>= 1) {
-                    A += __shfl_xor_sync(0xffffffffu, A, m);
-                    B += __shfl_xor_sync(0xffffffffu, B, m);
-                }
-            }
-            __syncthreads();                       // red_* reused by the next point
-        }
+    }
 
-        // H7: finalise and store (coalesced across the warp in the THREAD schedule)
-        if (lane == 0) {
-            const double mean_g = (double)acc.K + A * inv_n;
-            double m2 = ::fma(-A * inv_n, A, B);
-            m2 = m2 > 0.0 ? m2 : 0.0;
-            const double mean = p.volume * mean_g;
-            const double serr = p.volume * sqrt(m2 / ((double)(n - 1) * (double)n));
-            const uint64_t o = t - p.out_base;
-            if (p.out_f32) {
-                static_cast<float*>(out_mean)[o] = (float)mean;
-                static_cast<float*>(out_stderr)[o] = (float)serr;
-            } else {
-                static_cast<double*>(out_mean)[o] = mean;
-                static_cast<double*>(out_stderr)[o] = serr;
-            }
+    // H7: finalise and store (coalesced across the warp in the THREAD schedule)
+    if (lane == 0) {
+        const double mean_g = (double)acc.K + A * inv_n;
+        double m2 = ::fma(-A * inv_n, A, B);
+        m2 = m2 > 0.0 ? m2 : 0.0;
+        const double mean = p.volume * mean_g;
+        const double serr = p.volume * sqrt(m2 / ((double)(n - 1) * (double)n));
+        const uint64_t o = p.out_off + local;
+        if (p.out_f32) {
+            static_cast<float*>(out_mean)[o] = (float)mean;
+            static_cast<float*>(out_stderr)[o] = (float)serr;
+        } else {
+            static_cast<double*>(out_mean)[o] = mean;
+            static_cast<double*>(out_stderr)[o] = serr;
         }
-
-        // advance the digits by the worker stride (32-bit carries, no division)
-        uint32_t carry = 0;
-#pragma unroll
-        for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
-            if (i < M) {
-                uint32_t v = digit[i] + p.stride_digits[i] + carry;
-                carry = v >= p.counts[i] ? 1u : 0u;
-                digit[i] = v - (carry ? p.counts[i] : 0u);
-            }
-        }
-        digit[0] += p.stride_digits[0] + carry;
     }
 }
 

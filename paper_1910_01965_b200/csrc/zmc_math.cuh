@@ -40,30 +40,45 @@ struct PhiloxPoint {
         r2_e0 = r1_c1 ^ rk[2];                                    // c1 ^ k0 (then ^ hi1)
     }
 
-    __device__ __forceinline__ void block(uint32_t j, const uint32_t* __restrict__ rk,
-                                          uint32_t (&out)[4]) const {
-        // round 1: only word 0 (= j) varies
-        uint64_t p0 = (uint64_t)kPhiloxM0 * j;
-        uint32_t c2 = (uint32_t)(p0 >> 32) ^ r1_x;
-        uint32_t c3 = (uint32_t)p0;
-        // round 2: word 0 is invariant
-        uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
-        uint32_t c0 = (uint32_t)(p1 >> 32) ^ r2_e0;
-        uint32_t c1 = (uint32_t)p1;
-        c2 = r2_e2 ^ c3;
-        c3 = r2_c3;
+    // NBLK consecutive blocks j0 .. j0+NBLK-1 in lock-step (round by round), so that 2*NBLK independent
+    // multiplies are in flight: the IMAD.WIDE (fmaheavy) pipe, not the dependent chain, sets the pace.
+    template <int NBLK>
+    __device__ __forceinline__ void blocks(uint32_t j0, const uint32_t* __restrict__ rk, uint32_t* __restrict__ out) const {
+        uint32_t c0[NBLK], c1[NBLK], c2[NBLK], c3[NBLK];
+#pragma unroll
+        for (int b = 0; b < NBLK; ++b) {
+            // round 1: only word 0 (= j) varies
+            const uint64_t p0 = (uint64_t)kPhiloxM0 * (j0 + (uint32_t)b);
+            const uint32_t t2 = (uint32_t)(p0 >> 32) ^ r1_x;
+            // round 2: word 0 is invariant
+            const uint64_t p1 = (uint64_t)kPhiloxM1 * t2;
+            c0[b] = (uint32_t)(p1 >> 32) ^ r2_e0;
+            c1[b] = (uint32_t)p1;
+            c2[b] = r2_e2 ^ (uint32_t)p0;
+            c3[b] = r2_c3;
+        }
 #pragma unroll
         for (int r = 2; r < 10; ++r) {
-            p0 = (uint64_t)kPhiloxM0 * c0;
-            p1 = (uint64_t)kPhiloxM1 * c2;
-            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
-            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
-            c1 = (uint32_t)p1;
-            c3 = (uint32_t)p0;
-            c0 = n0;
-            c2 = n2;
+#pragma unroll
+            for (int b = 0; b < NBLK; ++b) {
+                const uint64_t p0 = (uint64_t)kPhiloxM0 * c0[b];
+                const uint64_t p1 = (uint64_t)kPhiloxM1 * c2[b];
+                const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1[b] ^ rk[2 * r];
+                const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3[b] ^ rk[2 * r + 1];
+                c1[b] = (uint32_t)p1;
+                c3[b] = (uint32_t)p0;
+                c0[b] = n0;
+                c2[b] = n2;
+            }
         }
-        out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+#pragma unroll
+        for (int b = 0; b < NBLK; ++b) {
+            out[4 * b + 0] = c0[b]; out[4 * b + 1] = c1[b]; out[4 * b + 2] = c2[b]; out[4 * b + 3] = c3[b];
+        }
+    }
+
+    __device__ __forceinline__ void block(uint32_t j, const uint32_t* __restrict__ rk, uint32_t (&out)[4]) const {
+        blocks<1>(j, rk, out);
     }
 };
 

@@ -7,9 +7,10 @@
 namespace zmc {
 
 struct ScanParams {
-    uint64_t first, end;          // flat indices [first, end) of this launch (GLOBAL indices, reading S3)
-    uint64_t out_base;            // element written = t - out_base
-    uint64_t stride;              // points between two consecutive points of one worker
+    uint64_t first;               // GLOBAL flat index (reading S3) of local point 0 of this launch
+    uint64_t out_off;             // element written = out_off + local point index
+    uint32_t count;               // points of this launch (<= 2^30: local indices and the grid stay 32-bit)
+    uint32_t base_digits[ZMC_MAX_M];    // mixed-radix digits of `first` (host-computed, 64-bit clean)
     const double* lists;          // device: the M value lists, concatenated
     uint32_t rk[20];              // Philox round keys: rk[2r] = k0 + r*W0, rk[2r+1] = k1 + r*W1
     uint32_t n;                   // samples per point
@@ -19,7 +20,6 @@ struct ScanParams {
     uint32_t out_f32;             // 1: outputs are float
     uint32_t counts[ZMC_MAX_M];   // list lengths L_i
     uint32_t list_off[ZMC_MAX_M]; // offset of list i in `lists`
-    uint32_t stride_digits[ZMC_MAX_M];  // mixed-radix digits of `stride` (top digit unbounded)
     double a[ZMC_MAX_N], width[ZMC_MAX_N];   // box; in F32E mode already rounded to float (mirror, reading S5)
     double volume;                // prod_k width_k, k ascending
     double consts[ZMC_MAX_CONSTS];
