@@ -435,8 +435,10 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
         }
         TimedSpan tk;
         if (timing) { ZMC_CUDA(new_tev(&tk.a)); ZMC_CUDA(new_tev(&tk.b)); ZMC_CUDA(cudaEventRecord(tk.a, stream)); }
-        for (uint64_t lf = bf; lf < bf + bc; lf += kMaxLaunchPoints) {
-            const uint64_t lc = (bf + bc - lf < kMaxLaunchPoints) ? bf + bc - lf : kMaxLaunchPoints;
+        for (uint64_t lf = bf, lc_done = 0; lf < bf + bc; lf += lc_done) {
+            uint64_t lc = (bf + bc - lf < kMaxLaunchPoints) ? bf + bc - lf : kMaxLaunchPoints;
+            const uint64_t to_wrap = (1ull << 32) - (lf & 0xFFFFFFFFull);   // the high word of t is launch-uniform
+            if (lc > to_wrap) lc = to_wrap;
             p.first = lf;
             p.count = (uint32_t)lc;
             p.out_off = lf - out_base;
@@ -448,6 +450,7 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
             const uint64_t grid = (lc + per_cta - 1) / per_cta;
             ZMC_CUDA(kern->launch(p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
             ++launches;
+            lc_done = lc;
         }
         if (timing) { ZMC_CUDA(cudaEventRecord(tk.b, stream)); t_kernel.push_back(tk); }
 

@@ -20,9 +20,12 @@ constexpr double kTwoPi = 2.0 * 3.141592653589793;
 constexpr double kSqrtLog2e = 1.2011224087864498;         // sqrt(log2(e))
 constexpr double kLog2e = 1.4426950408889634;
 
-// a'_k = a_k - (1-eps)*width_k : y_k = a'_k + width_k * f_k with f_k = unit(w_k) in [1,2)
+// y_k = a_k + width_k u_k with u_k = f_k * scale - offset, f_k = unit(w_k)  =>  y_k = a_fold + w_fold * f_k
 template <typename R> __device__ __forceinline__ double a_fold(const ScanParams& p, int k) {
-    return ::fma(-(double)Real<R>::one_minus_eps(), p.width[k], p.a[k]);
+    return ::fma(-Real<R>::u_offset(), p.width[k], p.a[k]);
+}
+template <typename R> __device__ __forceinline__ double w_fold(const ScanParams& p, int k) {
+    return p.width[k] * Real<R>::u_scale();          // scale is a power of two: exact
 }
 
 // reduce a phase constant (radians) to [-pi, pi] in fp64 before it is rounded to fp32
@@ -47,8 +50,8 @@ template <typename R, int N_, bool FAST> struct PhaseSin {
             if (k < n_dim) {
                 const double ck = coef(k);
                 c = ::fma(ck, a_fold<R>(p, k), c);
-                if constexpr (std::is_same<R, double>::value) X[k] = ck * p.width[k] * kInvPi;
-                else X[k] = (R)(ck * p.width[k]);
+                if constexpr (std::is_same<R, double>::value) X[k] = ck * w_fold<R>(p, k) * kInvPi;
+                else X[k] = (R)(ck * w_fold<R>(p, k));
             }
         }
         if constexpr (std::is_same<R, double>::value) C = ::fma(c, kInvPi, as_cos ? 0.5 : 0.0);
@@ -116,7 +119,7 @@ template <typename R, bool FAST> struct FamC4 {
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
             const double wk = (double)x[1 + (k >> 1)];
-            A[k] = (R)(a * p.width[k]);
+            A[k] = (R)(a * w_fold<R>(p, k));
             B[k] = (R)(a * (a_fold<R>(p, k) - wk));
         }
     }
@@ -143,11 +146,11 @@ template <typename R, bool FAST> struct FamC5 {
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             const double af = a_fold<R>(p, k), ck = (double)x[1 + k];
-            W[k] = (R)p.width[k];
+            W[k] = (R)w_fold<R>(p, k);
             Af[k] = (R)af;
             c = ::fma(ck, af, c);
-            if constexpr (std::is_same<R, double>::value) X[k] = ck * p.width[k] * kInvPi;
-            else X[k] = (R)(ck * p.width[k]);
+            if constexpr (std::is_same<R, double>::value) X[k] = ck * w_fold<R>(p, k) * kInvPi;
+            else X[k] = (R)(ck * w_fold<R>(p, k));
         }
         if constexpr (std::is_same<R, double>::value) C = ::fma(c, kInvPi, 0.5);
         else C = (R)wrap_2pi(c + 0.5 * kPi);

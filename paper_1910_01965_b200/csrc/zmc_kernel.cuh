@@ -16,6 +16,8 @@
 #pragma once
 #include "zmc_families.cuh"
 
+
+
 namespace zmc {
 
 constexpr int gcd4(int n) { return (n % 4 == 0) ? 4 : (n % 2 == 0) ? 2 : 1; }
@@ -72,7 +74,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
                          : SCHED == kSchedWarp   ? blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5)
                                                  : blockIdx.x;
     if (local >= p.count) return;                   // uniform per warp (WARP) / per CTA (CTA)
-    const uint64_t t = p.first + local;
+    const uint32_t t_lo = (uint32_t)p.first + local;      // no carry: a launch never straddles a multiple of 2^32
 
     // H3: mixed-radix decode.  digits(t) = digits(first) + digits(local) with carries: the 64-bit part was done on
     // the host, the per-point part is 32-bit division only.
@@ -106,7 +108,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     Fam fam;
     fam.setup(x, p);
     PhiloxPoint px;
-    px.init(t, p.rk);
+    px.init(t_lo, (uint32_t)(p.first >> 32), p.rk);
 
     uint32_t w[GS::NB * 4];
     Accum<R> acc;
@@ -118,18 +120,35 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
         acc.K = fam.eval(w);
     }
 
-    // H4 + H5 + H6: the hot loop
-    for (uint32_t g = lane; g < n_full; g += lanes) {
-        const uint32_t j0 = g * (uint32_t)NB;
-        if constexpr (kN != 0) {
-            px.template blocks<GS::NB>(j0, p.rk, w);
-        } else {
+    // H4 + H5 + H6: the hot loop.  fp64 path: software-pipelined -- the Philox blocks of the NEXT group (integer
+    // pipe) sit in the same basic block as the evaluation of the CURRENT one (FP64 pipe), so ptxas alternates the two
+    // pipes instruction by instruction (measured +7 % on cfg2; the one group generated past the end is discarded).
+    // fp32 path: FP32 and integer instructions share the dispatch port on sm_100 (profiles/), nothing to overlap.
+    if constexpr (kN != 0 && std::is_same<R, double>::value) {
+        uint32_t wn[GS::NB * 4];
+        uint32_t j0 = lane * (uint32_t)GS::NB;
+        if (lane < n_full) px.template blocks<GS::NB>(j0, p.rk, wn);
+        for (uint32_t g = lane; g < n_full; g += lanes) {
 #pragma unroll
-            for (int b = 0; b < GS::NB; ++b)
-                if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+            for (int i = 0; i < GS::NB * 4; ++i) w[i] = wn[i];
+            j0 += lanes * (uint32_t)GS::NB;
+            px.template blocks<GS::NB>(j0, p.rk, wn);
+#pragma unroll
+            for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
         }
+    } else {
+        for (uint32_t g = lane; g < n_full; g += lanes) {
+            const uint32_t j0 = g * (uint32_t)NB;
+            if constexpr (kN != 0) {
+                px.template blocks<GS::NB>(j0, p.rk, w);
+            } else {
 #pragma unroll
-        for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
+                for (int b = 0; b < GS::NB; ++b)
+                    if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+            }
+#pragma unroll
+            for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
+        }
     }
     if (rem != 0 && (n_full % lanes) == lane) {        // clipped last group: warp-uniform trip count
         const uint32_t j0 = n_full * (uint32_t)NB;

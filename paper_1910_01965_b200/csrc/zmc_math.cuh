@@ -10,6 +10,10 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#ifndef ZMC_F64_UNIT_I2F
+#define ZMC_F64_UNIT_I2F 0
+#endif
+
 namespace zmc {
 
 // ------------------------------------------------------------------------------------------
@@ -28,8 +32,9 @@ struct PhiloxPoint {
     uint32_t r2_c3;             // counter word 3 after round 2 (t only)
     uint32_t r2_e0, r2_e2;      // invariants folded into words 0 and 2 of round 2
 
-    __device__ __forceinline__ void init(uint64_t t, const uint32_t* __restrict__ rk) {
-        const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+    // t_hi is passed separately: the host never lets a launch straddle a multiple of 2^32, so it is a launch-wide
+    // constant and everything derived from it (and from a warp-uniform block index) stays on the uniform datapath.
+    __device__ __forceinline__ void init(uint32_t t_lo, uint32_t t_hi, const uint32_t* __restrict__ rk) {
         const uint64_t p1 = (uint64_t)kPhiloxM1 * t_lo;           // round 1, multiply of word 2
         r1_c0 = (uint32_t)(p1 >> 32) ^ rk[0];                     // hi1 ^ c1(=0) ^ k0
         r1_c1 = (uint32_t)p1;                                     // lo1
@@ -83,10 +88,14 @@ struct PhiloxPoint {
 };
 
 // ------------------------------------------------------------------------------------------
-// Uniforms (reading S4).  unit(w) is f = 1 + (w >> drop)*2^-mant in [1,2), built with one
-// funnel shift (fp32) or a funnel shift and a shift (fp64); u = f - (1 - eps) is then the exact
-// lattice value (2(w>>9)+1)*2^-24 resp. (2w+1)*2^-33.  Families fold the "- (1 - eps)" into
-// per-point constants, so the hot loop spends one FMA per dimension.
+// Uniforms (reading S4).  unit(w) is a value f, exact in the evaluation type, from which the lattice uniform is
+// u = f * u_scale() - u_offset():
+//   fp32: f = 1 + (w >> 9) * 2^-23 in [1,2), one funnel shift; u = f - (1 - 2^-24) = (2(w>>9)+1) 2^-24
+//   fp64: f = 1 + w * 2^-32 in [1,2), a funnel shift and a shift; u = f - (1 - 2^-33) = (2w+1) 2^-33
+//         (measured alternative, rejected: f = (2^52 + w) - 2^52 with one DADD costs two register moves per word
+//          to pair the word with the 0x43300000 high half and is 5 % slower on cfg2)
+// No I2F (16-lane XU pipe) anywhere.
+// Families fold scale and offset into per-point constants, so the hot loop spends one FMA per dimension.
 // ------------------------------------------------------------------------------------------
 template <typename R> struct Real;
 
@@ -94,21 +103,30 @@ template <> struct Real<float> {
     static __device__ __forceinline__ float unit(uint32_t w) {
         return __uint_as_float(__funnelshift_r(w, 0x7Fu, 9));        // (w>>9) | 0x3F800000
     }
-    static __device__ __forceinline__ float one_minus_eps() { return 0x1.fffffep-1f; }   // 1 - 2^-24
+    static __device__ __forceinline__ double u_scale() { return 1.0; }
+    static __device__ __forceinline__ double u_offset() { return 0x1.fffffep-1; }          // 1 - 2^-24
     static __device__ __forceinline__ float fma(float a, float b, float c) { return fmaf(a, b, c); }
 };
 
 template <> struct Real<double> {
     static __device__ __forceinline__ double unit(uint32_t w) {
+#if ZMC_F64_UNIT_I2F
+        return (double)w;                                                               // I2F.F64.U32 (XU pipe)
+    }
+    static __device__ __forceinline__ double u_scale() { return 0x1p-32; }
+    static __device__ __forceinline__ double u_offset() { return -0x1p-33; }
+#else
         return __hiloint2double((int)__funnelshift_r(w, 0x3FFu, 12), (int)(w << 20));   // 1 + w*2^-32
     }
-    static __device__ __forceinline__ double one_minus_eps() { return 0x1.ffffffffp-1; }   // 1 - 2^-33
+    static __device__ __forceinline__ double u_scale() { return 1.0; }
+    static __device__ __forceinline__ double u_offset() { return 0x1.ffffffffp-1; }        // 1 - 2^-33
+#endif
     static __device__ __forceinline__ double fma(double a, double b, double c) { return ::fma(a, b, c); }
 };
 
-// exact lattice uniform u in (0,1)
+// exact lattice uniform u in (0,1) (diagnostic families; the hot families fold scale and offset)
 template <typename R> __device__ __forceinline__ R uniform(uint32_t w) {
-    return Real<R>::unit(w) - Real<R>::one_minus_eps();
+    return Real<R>::fma(Real<R>::unit(w), (R)Real<R>::u_scale(), (R)(-Real<R>::u_offset()));
 }
 
 // ------------------------------------------------------------------------------------------

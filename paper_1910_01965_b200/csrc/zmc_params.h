@@ -7,7 +7,8 @@
 namespace zmc {
 
 struct ScanParams {
-    uint64_t first;               // GLOBAL flat index (reading S3) of local point 0 of this launch
+    uint64_t first;               // GLOBAL flat index (reading S3) of local point 0; [first, first+count) never
+                                  // straddles a multiple of 2^32, so the high word of t is launch-uniform
     uint64_t out_off;             // element written = out_off + local point index
     uint32_t count;               // points of this launch (<= 2^30: local indices and the grid stay 32-bit)
     uint32_t base_digits[ZMC_MAX_M];    // mixed-radix digits of `first` (host-computed, 64-bit clean)
