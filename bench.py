@@ -8,7 +8,7 @@ reduce, finalise, store) over one synthetic workload of BASELINE.json `configs` 
 configs[1] = cfg2; cfg5 streams its 80 GB of results to pinned host memory).  `value` is
 integrand evaluations/s with device-resident outputs; `e2e` is the same metric through the C ABI
 with HOST output buffers (list H2D and result D2H inside the timed region).  `roofline` is the
-instruction-issue bound of DESIGN.md ("bound": "alu"); `cpu_baseline` is the CPU oracle, as it
+measured-dispatch-cost ALU bound of DESIGN.md section 6 ("bound": "alu"); `cpu_baseline` is the CPU oracle, as it
 stands, on a bounded sample of the same workload.  With N > 1 (torchrun) the grid's first list is
 lengthened N-fold and each rank scans its own contiguous flat range -- no data-path collective.
 """
@@ -32,11 +32,32 @@ from paper_1910_01965_b200 import workloads as wl  # noqa: E402
 METRIC = "integrand_evals_per_s"
 UNIT = "evals/s"
 
-# Algorithmic thread-instructions per integrand evaluation (Philox blocks +
-# uniform bit ops + one FMA per dimension + the family's arithmetic + the fp64 accumulate).
-I_MIN = {"cfg1": 30.25, "cfg2": 42.5, "cfg3": 51.0, "cfg4": 78.5, "cfg5": 52.75}
-SM_COUNT, ISSUE_PER_SM_CLK, SM_MAX_MHZ = 148, 128, 1965.0
-PEAK_GINSTR = SM_COUNT * ISSUE_PER_SM_CLK * SM_MAX_MHZ * 1e6 / 1e9      # 37 228.8 G thread-instr/s
+# ALU roofline.  The loop is bound by the SM sub-partition's dispatch of half-width (16-lane)
+# pipes, measured by `python -m paper_1910_01965_b200.pipe_rates` (profiles/r01_pipe_rates.txt): every integer
+# instruction (IMAD.WIDE, LOP3, SHF, IADD3) costs 2 SMSP-cycles per warp, every FP32 instruction 1, and the two
+# classes serialise on one port ("main"); FP64 instructions cost 2 on their own pipe, MUFU and F2F 8 each on the XU pipe.
+# W_MIN[cfg] = max over those resources of the ALGORITHMIC instruction list of one evaluation (Philox4x32-10 with the
+# t-only rounds hoisted = 16 IMAD.WIDE + 18 LOP3 per block, one bit-op per uniform (two for fp64), one FMA per
+# dimension, the integrand's own arithmetic, F2F + 2 fp64 accumulate ops), in SMSP-cycles per warp = lane-cycles per
+# thread.  (int ops, fp32 ops, fp64 ops, MUFU, F2F) per evaluation:
+ALG_OPS = {
+    "cfg1": (0.25 * 34 + 2 + 2, 0, 1 + 13 + 3, 0, 0),     # fp64 cos via sinpi: 13 fp64 + 2 int (sign)
+    "cfg2": (0.50 * 34 + 4 + 2, 0, 2 + 13 + 3, 0, 0),
+    "cfg3": (1.00 * 34 + 4, 4 + 2, 2, 1, 1),              # 4 FFMA + FMUL(1/2pi) + FADD(shift); MUFU.SIN
+    "cfg4": (1.50 * 34 + 6, 12 + 1, 2, 1, 1),             # 2 FFMA per dimension + FADD; MUFU.EX2
+    "cfg5": (0.75 * 34 + 3, 17, 2, 2, 1),                 # 17 FP32 ops; MUFU.SIN + MUFU.EX2
+}
+
+
+def w_min(name):
+    i, f, d, mufu, f2f = ALG_OPS[name]
+    res = {"main(int*2+fp32)": 2 * i + f, "fp64": 2 * d, "xu": 8 * mufu + 8 * f2f, "issue": i + f + d + mufu + f2f}
+    bound = max(res, key=res.get)
+    return res[bound], bound, res
+
+
+SM_COUNT, LANES_PER_SM_CLK, SM_MAX_MHZ = 148, 128, 1965.0
+PEAK_GLANE = SM_COUNT * LANES_PER_SM_CLK * SM_MAX_MHZ * 1e6 / 1e9      # 37 225 G lane-cycles/s
 
 
 def build_workload(name: str, world: int):
@@ -129,7 +150,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2", choices=sorted(I_MIN))
+    ap.add_argument("--workload", default="cfg2", choices=sorted(ALG_OPS))
     ap.add_argument("--impl", default="zmc", choices=["zmc", "reference"])
     ap.add_argument("--schedule", type=int, default=0, help="0 auto, 1 thread, 2 warp, 3 cta")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -244,8 +265,8 @@ def main():
             dist.destroy_process_group()
         return
 
-    i_min = I_MIN[w.name]
-    achieved = i_min * evals_rank / (kernel_ms * 1e-3) / 1e9
+    w_cyc, w_bound, w_res = w_min(w.name)
+    achieved = w_cyc * evals_rank / (kernel_ms * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -259,11 +280,14 @@ def main():
         "clocks": clocks,
         "e2e": e2e,
         "gpu_launches": launches,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GINSTR, "unit": "G thread-instr/s",
-                     "frac": achieved / PEAK_GINSTR, "traffic": None,
-                     "i_min_per_eval": i_min,
-                     "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1965 MHz (DESIGN.md; issue-bound)",
-                     "frac_at_measured_clock": (achieved / (PEAK_GINSTR * clocks["sm_mhz"] / SM_MAX_MHZ)
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
+                     "frac": achieved / PEAK_GLANE, "traffic": None,
+                     "lane_cycles_per_eval": w_cyc, "binding_resource": w_bound, "resources": w_res,
+                     "measured_lane_cycles_per_eval": PEAK_GLANE * 1e9 * (clocks["sm_mhz"] or SM_MAX_MHZ) / SM_MAX_MHZ
+                     / (evals_rank / (kernel_ms * 1e-3)),
+                     "peak_source": "148 SMs x 4 SMSPs x 32 lanes x 1965 MHz dispatch; per-class costs measured by "
+                                    "paper_1910_01965_b200.pipe_rates (profiles/r01_pipe_rates.txt), DESIGN.md section 6",
+                     "frac_at_measured_clock": (achieved / (PEAK_GLANE * clocks["sm_mhz"] / SM_MAX_MHZ)
                                                 if clocks.get("sm_mhz") else None)},
     }
     if not args.no_cpu_baseline and world == 1:

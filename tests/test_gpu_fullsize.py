@@ -1,0 +1,112 @@
+"""-m gpu: the BASELINE.json configs at FULL size, in the launch configuration bench.py times (AUTO schedule,
+the workload's own batch size and output placement), checked on sampled outputs the CPU oracle computes one by
+one (reading Q17 of DESIGN.md: seeded random subset + forced edge points), plus properties that hold at any size.
+
+Tolerances are the ones of tests/test_gpu_parity.py (north_star; reading Q12).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import zmc_oracle as orc
+from paper_1910_01965_b200 import workloads as wl
+import closed_forms as cf
+
+pytestmark = pytest.mark.gpu
+NT = min(16, os.cpu_count() or 1)
+
+
+def q17_indices(G, n_random, batch_points):
+    """t_r = (R0 + 2^32 R1) mod G with R = Philox(ctr=(r,0,0,0), key=(0x5EED,0)) (the oracle's own Philox),
+    plus the forced points 0, G-1, batch edges, 2^32-1, 2^32, 2^33."""
+    idx = []
+    for ctr, key in wl.subset_indices_seed_words(n_random):
+        r = orc.philox(ctr, key)
+        idx.append((r[0] + (r[1] << 32)) % G)
+    idx += wl.forced_indices(G, batch_points)
+    return np.array(sorted(set(idx)), dtype=np.uint64)
+
+
+def check(w, mean, err, idx):
+    rc, mean_o, err_o = orc.points_workload(w, idx, n_threads=NT)
+    assert rc == 0
+    m = np.asarray(mean)[idx.astype(np.int64)].astype(np.float64)      # index first: `mean` may hold 10^10 elements
+    e = np.asarray(err)[idx.astype(np.int64)].astype(np.float64)
+    if w.precision == wl.PREC_F64:
+        bad_m = np.abs(m - mean_o) > 1e-10 * np.maximum(np.abs(mean_o), err_o)
+        bad_e = np.abs(e - err_o) > 1e-10 * err_o
+    else:
+        bad_m = np.abs(m - mean_o) > 1e-4 * np.abs(mean_o) + 1e-6
+        bad_e = np.abs(e - err_o) > 1e-4 * np.abs(err_o) + 1e-6
+    assert not bad_m.any(), f"mean: {bad_m.sum()} of {len(idx)} sampled points off"
+    assert not bad_e.any(), f"stderr: {bad_e.sum()} of {len(idx)} sampled points off"
+    return mean_o, err_o
+
+
+def gpu_scan(w, **kw):
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    m, e, tm = zb.scan_workload(w, timing=True, **kw)
+    torch.cuda.synchronize()
+    return (m.cpu().numpy() if m.is_cuda else m.numpy()), (e.cpu().numpy() if e.is_cuda else e.numpy()), tm
+
+
+def test_cfg1_full_grid_every_point():
+    w = wl.config(1)
+    mean, err, tm = gpu_scan(w)
+    mean_o, err_o = check(w, mean, err, np.arange(w.G, dtype=np.uint64))
+    x = w.lists[0]
+    z = (mean - cf.c1_mean(x)) / err          # closed form sin(x1)/x1: 5-sigma coverage on the GPU result itself
+    assert np.mean(np.abs(z) <= 5) >= 0.999
+
+
+def test_cfg2_full_size_sampled():
+    w = wl.config(2)
+    mean, err, tm = gpu_scan(w)
+    assert tm["n_batches"] == 1 and len(mean) == w.G
+    check(w, mean, err, q17_indices(w.G, 20_000, 0))
+    assert np.isfinite(mean).all() and (err > 0).all()
+    # property at any size: the grid of sin(x1 y1 + x2 y2) on a symmetric pair of lists is symmetric in expectation;
+    # the estimates at (i, j) and (j, i) use different streams, so they agree within their standard errors
+    g = mean.reshape(1000, 1000)
+    s = np.sqrt(err.reshape(1000, 1000) ** 2 + err.reshape(1000, 1000).T ** 2)
+    assert np.mean(np.abs(g - g.T) <= 5 * s) >= 0.999
+
+
+def test_cfg3_full_size_sampled():
+    w = wl.config(3)
+    mean, err, tm = gpu_scan(w)
+    assert len(mean) == w.G
+    check(w, mean, err, q17_indices(w.G, 100_000, 0))
+    assert np.isfinite(mean).all() and np.isfinite(err).all()
+
+
+def test_cfg4_full_size_sampled():
+    w = wl.config(4)
+    mean, err, tm = gpu_scan(w)
+    assert len(mean) == w.G
+    check(w, mean, err, q17_indices(w.G, 200_000, 0))
+    assert np.isfinite(mean).all() and (mean >= 0).all() and (mean <= 1.0 + 1e-6).all()     # 0 < g <= 1, V = 1
+
+
+def test_cfg5_full_size_streamed_to_pinned_host():
+    """10^10 points, 38 batches of 2^28 streamed to 80 GB of pinned host memory with D2H on the side stream."""
+    import torch
+    w = wl.config(5)
+    try:
+        mean = torch.empty(w.G, dtype=torch.float32, pin_memory=True)
+        err = torch.empty(w.G, dtype=torch.float32, pin_memory=True)
+    except RuntimeError as exc:
+        pytest.skip(f"cannot pin 80 GB of host memory on this box: {exc}")
+    mean.fill_(float("nan")); err.fill_(float("nan"))
+    m, e, tm = gpu_scan(w, out_mean=mean, out_stderr=err)
+    assert tm["n_batches"] == 38 and tm["d2h_bytes"] == 8 * w.G
+    idx = q17_indices(w.G, 100_000, w.batch_points)
+    assert idx.max() == w.G - 1 and (1 << 32) in set(idx.tolist())
+    check(w, m, e, idx)
+    # every element was written (no NaN left), sampled in strides to keep the host pass short
+    assert not np.isnan(m[::997]).any() and not np.isnan(e[::997]).any()
+    # D2H hidden behind compute (north_star): what is exposed is at most the last batch's copy plus launch gaps
+    last_copy_ms = tm["d2h_ms"] / tm["n_batches"] * 1.5
+    assert tm["exposed_d2h_ms"] <= last_copy_ms + 5.0, tm
