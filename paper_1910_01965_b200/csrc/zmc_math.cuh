@@ -153,21 +153,33 @@ __device__ __forceinline__ double sinpi_f64(double z) {
     return __hiloint2double(hi, __double2loint(v));
 }
 
-// Transcendentals of the evaluation type.  FAST selects the MUFU forms for fp32 (reading:
-// north_star "fast-math transcendentals only where the tolerance allows"); fp64 ignores it.
+// Transcendentals of the evaluation type.  FAST selects the MUFU forms for fp32 (north_star: "fast-math
+// transcendentals only where the tolerance allows"); fp64 ignores it.  Trig families keep their phase in the unit
+// kPhasePerRad * radians and call sin_phase():
+//   fp64          : units of pi      -> sinpi_f64 (exact range reduction)
+//   fp32 + MUFU   : turns (1/2pi)    -> r = ph - rint(ph) exactly, then sin.approx(2 pi r).  sin.approx scales its
+//                   argument with a round-toward-zero FMUL; on an unreduced phase of up to 60 rad that bias
+//                   (~ |ph| 2^-24 rad, same sign for every sample) exceeded the 1e-4 + 1e-6 tolerance at 0.01 % of
+//                   cfg 5's grid points; on |2 pi r| <= pi it is 15x smaller and odd-symmetric, so it averages out
+//   fp32 accurate : radians          -> sinf
 template <typename R, bool FAST> struct Fn;
 
 template <bool FAST> struct Fn<double, FAST> {
-    // arguments are phases in units of pi ("turns/2"): families pre-scale their coefficients by 1/pi
-    static __device__ __forceinline__ double sin_pi(double z) { return sinpi_f64(z); }
+    static constexpr double kPhasePerRad = 0.31830988618379067154;       // 1/pi
+    static constexpr double kQuarter = 0.5;                              // pi/2 in phase units
+    static __device__ __forceinline__ double wrap(double c) { return c; }
+    static __device__ __forceinline__ double sin_phase(double z) { return sinpi_f64(z); }
     static __device__ __forceinline__ double exp2_neg(double e) { return ::exp2(-e); }
-    static constexpr bool kPhaseInPi = true;
 };
 
 template <> struct Fn<float, true> {
-    // phase in radians: sin.approx = FMUL(1/2pi) + MUFU.SIN
-    static __device__ __forceinline__ float sin_rad(float a) { return __sinf(a); }
-    static __device__ __forceinline__ float cos_rad(float a) { return __cosf(a); }
+    static constexpr double kPhasePerRad = 0.15915494309189533577;       // 1/(2 pi)
+    static constexpr double kQuarter = 0.25;
+    static __device__ __forceinline__ double wrap(double c) { return c - rint(c); }
+    static __device__ __forceinline__ float sin_phase(float t) {
+        const float r = t - rintf(t);                                    // FRND (XU pipe) + FADD, exact
+        return __sinf(r * 6.283185307179586f);                           // FMUL, then FMUL.RZ(1/2pi) + MUFU.SIN
+    }
     static __device__ __forceinline__ float exp2_neg(float e) {            // 2^-e: one MUFU.EX2
         float r;
         asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-e));
@@ -176,8 +188,10 @@ template <> struct Fn<float, true> {
 };
 
 template <> struct Fn<float, false> {
-    static __device__ __forceinline__ float sin_rad(float a) { return sinf(a); }
-    static __device__ __forceinline__ float cos_rad(float a) { return cosf(a); }
+    static constexpr double kPhasePerRad = 1.0;
+    static constexpr double kQuarter = 1.5707963267948966;
+    static __device__ __forceinline__ double wrap(double c) { return c - 6.283185307179586 * rint(c * 0.15915494309189533577); }
+    static __device__ __forceinline__ float sin_phase(float a) { return sinf(a); }
     static __device__ __forceinline__ float exp2_neg(float e) { return exp2f(-e); }
 };
 
