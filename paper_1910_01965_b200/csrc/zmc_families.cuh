@@ -6,7 +6,8 @@
 //
 // Interface:  struct Fam { using real; static constexpr int kN (0 = runtime N);
 //                          void setup(const real* x, const ScanParams& p);   // once per point
-//                          real eval(const uint32_t* w) const; }             // w: the N words of one sample
+//                          real eval_shifted(const uint32_t* w, real K) const; // g - K; w: the N words of one sample
+//                          real eval(const uint32_t* w) const; }               // g (used once per point, for K)
 #pragma once
 #include <type_traits>
 #include "zmc_math.cuh"
@@ -61,8 +62,9 @@ template <typename R, int N_, bool FAST> struct PhaseSin {
         return ph;
     }
 
-    __device__ __forceinline__ R eval(const uint32_t* w) const {
-        return Fn<R, FAST>::sin_phase(phase(w));
+    __device__ __forceinline__ R eval(const uint32_t* w) const { return Fn<R, FAST>::sin_phase(phase(w)); }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const {
+        return Fn<R, FAST>::sin_phase_minus(phase(w), K);
     }
 };
 
@@ -126,6 +128,7 @@ template <typename R, bool FAST> struct FamC4 {
         }
         return Fn<R, FAST>::exp2_neg(acc);
     }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
 };
 
 // c5: exp(-x1 |y|^2) cos(x2 y0 + x3 y1 + x4 y2) (1 + x5 y0 y1 y2)      (configs[4])
@@ -149,7 +152,7 @@ template <typename R, bool FAST> struct FamC5 {
         damp = (R)((double)x[0] * kLog2e);
         x5 = x[4];
     }
-    __device__ __forceinline__ R eval(const uint32_t* w) const {
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const {
         const R f0 = Real<R>::unit(w[0]), f1 = Real<R>::unit(w[1]), f2 = Real<R>::unit(w[2]);
         const R y0 = Real<R>::fma(f0, W[0], Af[0]);
         const R y1 = Real<R>::fma(f1, W[1], Af[1]);
@@ -158,8 +161,9 @@ template <typename R, bool FAST> struct FamC5 {
         const R ph = Real<R>::fma(y2, X[2], Real<R>::fma(y1, X[1], Real<R>::fma(y0, X[0], C)));
         const R poly = Real<R>::fma(x5, y0 * y1 * y2, (R)1);
         const R osc = Fn<R, FAST>::sin_phase(ph);
-        return Fn<R, FAST>::exp2_neg(damp * r2) * osc * poly;
+        return Real<R>::fma(Fn<R, FAST>::exp2_neg(damp * r2) * osc, poly, -K);      // the shift rides in the last FMA
     }
+    __device__ __forceinline__ R eval(const uint32_t* w) const { return eval_shifted(w, (R)0); }
 };
 
 // ---- diagnostics (tests only): exact y_k = fma(u_k, width_k, a_k), no folding ---------------------
@@ -168,6 +172,7 @@ template <typename R> struct FamConstOne {
     static constexpr int kN = 0;
     __device__ __forceinline__ void setup(const R*, const ScanParams&) {}
     __device__ __forceinline__ R eval(const uint32_t*) const { return (R)1; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
 };
 
 template <typename R> struct FamParamEcho {
@@ -182,6 +187,7 @@ template <typename R> struct FamParamEcho {
             if (l == i) v = x[l];
     }
     __device__ __forceinline__ R eval(const uint32_t*) const { return v; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
 };
 
 template <typename R> struct FamLinY {
@@ -197,6 +203,7 @@ template <typename R> struct FamLinY {
     __device__ __forceinline__ R eval(const uint32_t* w) const {
         return Real<R>::fma(uniform<R>(w[k]), width, a);
     }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
 };
 
 template <typename R> struct FamPoly {
@@ -210,6 +217,7 @@ template <typename R> struct FamPoly {
             prod *= Real<R>::fma(uniform<R>(w[k]), (R)pp->width[k], (R)pp->a[k]);
         return prod;
     }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
 };
 
 }  // namespace zmc

@@ -35,10 +35,8 @@ template <> struct GroupShape<0> {     // runtime N: 4 samples = N blocks
 template <typename R> struct Accum {
     double A = 0.0, B = 0.0;
     R K;
-    __device__ __forceinline__ void add(R g) {
-        double d;
-        if constexpr (std::is_same<R, double>::value) d = g - K;
-        else d = (double)(g - K);          // fp32 subtract is exact when g ~ K (Sterbenz), else harmless
+    __device__ __forceinline__ void add_shifted(R d_) {     // d_ = g - K, formed in the evaluation type
+        const double d = (double)d_;                        // (fp32: exact when g ~ K by Sterbenz, else harmless)
         A += d;
         B = ::fma(d, d, B);
     }
@@ -134,7 +132,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
             j0 += lanes * (uint32_t)GS::NB;
             px.template blocks<GS::NB>(j0, p.rk, wn);
 #pragma unroll
-            for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
+            for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
         }
     } else {
         for (uint32_t g = lane; g < n_full; g += lanes) {
@@ -147,7 +145,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
                     if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
             }
 #pragma unroll
-            for (int s = 0; s < S; ++s) acc.add(fam.eval(&w[s * N]));
+            for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
         }
     }
     if (rem != 0 && (n_full % lanes) == lane) {        // clipped last group: warp-uniform trip count
@@ -157,7 +155,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
             if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
 #pragma unroll
         for (int s = 0; s < S - 1; ++s)
-            if ((uint32_t)s < rem) acc.add(fam.eval(&w[s * N]));
+            if ((uint32_t)s < rem) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
     }
 
     // H6: combine lanes (plain sums: the shift K is common to all lanes of the point)

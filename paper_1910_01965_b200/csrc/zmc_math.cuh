@@ -132,13 +132,17 @@ template <typename R> __device__ __forceinline__ R uniform(uint32_t w) {
 // ------------------------------------------------------------------------------------------
 // fp64 sin(pi z), any |z| < 2^51.  k = rint(z) by the magic-number add, r = z - k exact,
 // sin(pi z) = (-1)^k sin(pi r), |r| <= 1/2; odd polynomial r*P7(r^2), max error 2.4e-16
-// (Chebyshev-node fit of sin(pi sqrt(s))/sqrt(s) on [0,1/4]).  13 fp64-pipe ops + 2 ALU ops.
+// (Chebyshev-node fit of sin(pi sqrt(s))/sqrt(s) on [0,1/4]).
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ double sinpi_f64(double z) {
+// sinpi_minus_f64(z, K) = sin(pi z) - K: the sign is applied to r BEFORE the polynomial and the shift K of the
+// accumulator (reading S6) rides in the last FMA, so the whole thing is 12 fp64-pipe ops + 2 integer ops.
+__device__ __forceinline__ double sinpi_minus_f64(double z, double K) {
     const double kMagic = 6755399441055744.0;                  // 1.5 * 2^52
     const double kf = z + kMagic;
-    const double r = z - (kf - kMagic);
-    const double s = r * r;
+    const double r0 = z - (kf - kMagic);
+    // sign flip for odd k: xor bit 0 of k into the sign bit of r
+    const double r = __hiloint2double(__double2hiint(r0) ^ (__double2loint(kf) << 31), __double2loint(r0));
+    const double s = r0 * r0;
     double p = -0x1.62903d02bb153p-16;
     p = ::fma(p, s, 0x1.e89f6fe44fe7bp-12);
     p = ::fma(p, s, -0x1.e30631bdf732dp-8);
@@ -146,12 +150,10 @@ __device__ __forceinline__ double sinpi_f64(double z) {
     p = ::fma(p, s, -0x1.32d2cce1ea145p-1);
     p = ::fma(p, s, 0x1.466bc677522bdp+1);
     p = ::fma(p, s, -0x1.4abbce625bd83p+2);
-    const double rs = r * s;
-    const double v = ::fma(rs, p, r * 0x1.921fb54442d17p+1) ;
-    // sign flip for odd k: xor bit 0 of k into the sign bit
-    const int hi = __double2hiint(v) ^ (__double2loint(kf) << 31);
-    return __hiloint2double(hi, __double2loint(v));
+    p = ::fma(p, s, 0x1.921fb54442d18p+1);                     // pi
+    return ::fma(r, p, -K);
 }
+__device__ __forceinline__ double sinpi_f64(double z) { return sinpi_minus_f64(z, 0.0); }
 
 // Transcendentals of the evaluation type.  FAST selects the MUFU forms for fp32 (north_star: "fast-math
 // transcendentals only where the tolerance allows"); fp64 ignores it.  Trig families keep their phase in the unit
@@ -169,6 +171,7 @@ template <bool FAST> struct Fn<double, FAST> {
     static constexpr double kQuarter = 0.5;                              // pi/2 in phase units
     static __device__ __forceinline__ double wrap(double c) { return c; }
     static __device__ __forceinline__ double sin_phase(double z) { return sinpi_f64(z); }
+    static __device__ __forceinline__ double sin_phase_minus(double z, double K) { return sinpi_minus_f64(z, K); }
     static __device__ __forceinline__ double exp2_neg(double e) { return ::exp2(-e); }
 };
 
@@ -180,6 +183,7 @@ template <> struct Fn<float, true> {
         const float r = t - rintf(t);                                    // FRND (XU pipe) + FADD, exact
         return __sinf(r * 6.283185307179586f);                           // FMUL, then FMUL.RZ(1/2pi) + MUFU.SIN
     }
+    static __device__ __forceinline__ float sin_phase_minus(float t, float K) { return sin_phase(t) - K; }
     static __device__ __forceinline__ float exp2_neg(float e) {            // 2^-e: one MUFU.EX2
         float r;
         asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-e));
@@ -192,6 +196,7 @@ template <> struct Fn<float, false> {
     static constexpr double kQuarter = 1.5707963267948966;
     static __device__ __forceinline__ double wrap(double c) { return c - 6.283185307179586 * rint(c * 0.15915494309189533577); }
     static __device__ __forceinline__ float sin_phase(float a) { return sinf(a); }
+    static __device__ __forceinline__ float sin_phase_minus(float a, float K) { return sinf(a) - K; }
     static __device__ __forceinline__ float exp2_neg(float e) { return exp2f(-e); }
 };
 

@@ -56,6 +56,34 @@ template <int A, int NA, int B, int NB> __global__ void __launch_bounds__(256) m
     out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
+// three-class groups, interleaved round-robin: P x (IMAD.WIDE+LOP3), L x LOP3, D x DFMA -- the instruction mix of the
+// fp64 path (cfg 2 has 26 integer : 18 FP64 instructions per evaluation, i.e. P=1, L=1, D=2)
+template <int P, int L, int D> __global__ void __launch_bounds__(256) mix3(uint32_t* out, int iters, uint32_t k, double dk) {
+    uint32_t r[8], e[8]; double d[8];
+    for (int i = 0; i < 8; ++i) {
+        r[i] = threadIdx.x * 2654435761u + i * 40503u + k; e[i] = r[i] * 3u + 1u; d[i] = 1.0 + 1e-9 * (threadIdx.x + i);
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            constexpr int T = (P > L ? P : L) > D ? (P > L ? P : L) : D;
+#pragma unroll
+            for (int x = 0; x < T; ++x) {
+                if (x < P) {
+                    uint64_t p;
+                    asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(r[(u + x) & 7]), "n"(M0));
+                    asm volatile("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r[(u + x) & 7]) : "r"((uint32_t)p), "r"((uint32_t)(p >> 32)), "r"(k));
+                }
+                if (x < D) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(d[(u + x) & 7]) : "d"(dk), "d"(1e-3));
+                if (x < L) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(e[(u + x) & 7]) : "r"(k), "r"(e[(u + x + 1) & 7]));
+            }
+        }
+    }
+    uint32_t acc = 0;
+    for (int i = 0; i < 8; ++i) acc ^= r[i] ^ e[i] ^ (uint32_t)__double2loint(d[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 // Philox4x32-10 from its definition, counter (j, 0, t, 0): the compiler hoists what depends on t only
 __global__ void __launch_bounds__(256) philox_only(uint32_t* out, int n_blocks, uint32_t k0, uint32_t k1) {
     uint32_t rk[20];
@@ -103,6 +131,18 @@ template <int A, int NA, int B, int NB> void run_mix(uint32_t* out, bool quiet =
     cudaEventDestroy(a); cudaEventDestroy(b);
 }
 
+template <int P, int L, int D> void run_mix3(uint32_t* out) {
+    const int grid = g_sms * 8, iters = 2000;
+    mix3<P, L, D><<<grid, 256>>>(out, iters, 12345u, 0.999);
+    cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+    cudaEventRecord(a); mix3<P, L, D><<<grid, 256>>>(out, iters, 12345u, 0.999); cudaEventRecord(b); cudaEventSynchronize(b);
+    float ms; cudaEventElapsedTime(&ms, a, b);
+    const double warp_groups_per_smsp = 8.0 * iters * (256 / 32) * 8 / 4.0;
+    printf("%d x (IMAD.WIDE+LOP3) + %d x LOP3 + %d x DFMA : %6.2f SMSP-cycles per group  (bound: integer %d, fp64 %d, issue %d)\n", P, L, D,
+           ms * 1e-3 * g_mhz * 1e6 / warp_groups_per_smsp, 4 * P + 2 * L, 2 * D, 2 * P + L + D);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+}
+
 int main() {
     cudaDeviceProp prop; cudaGetDeviceProperties(&prop, 0); g_sms = prop.multiProcessorCount;
     uint32_t* out; cudaMalloc(&out, (size_t)g_sms * 8 * 256 * 4 * 4);
@@ -120,6 +160,7 @@ int main() {
     run_mix<DFMA, 1, LOP3, 1>(out); run_mix<DFMA, 2, LOP3, 2>(out); run_mix<DFMA, 4, LOP3, 4>(out); run_mix<DFMA, 1, LOP3, 2>(out);
     run_mix<MUFU, 1, LOP3, 2>(out); run_mix<MUFU, 1, LOP3, 4>(out); run_mix<MUFU, 1, LOP3, 8>(out);
     run_mix<F2F, 1, LOP3, 2>(out); run_mix<F2F, 1, LOP3, 4>(out);
+    run_mix3<1, 0, 1>(out); run_mix3<1, 0, 2>(out); run_mix3<1, 1, 2>(out); run_mix3<2, 3, 4>(out); run_mix3<0, 3, 2>(out);
     {
         const int grid = g_sms * 32, n_blocks = 4000;
         philox_only<<<grid, 256>>>(out, 16, 1u, 0u);
