@@ -1,0 +1,98 @@
+"""-m gpu: edge cases of the CUDA path against the CPU oracle -- empty and ragged inputs, smallest and largest
+shapes the boundary accepts, degenerate grids, lists too long for shared-memory staging."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import zmc_oracle as orc
+from paper_1910_01965_b200 import workloads as wl
+from test_gpu_parity import assert_parity, run_gpu
+
+pytestmark = pytest.mark.gpu
+NT = min(16, os.cpu_count() or 1)
+
+
+def _check(w, **kw):
+    first, count = kw.get("first_index", 0), kw.get("count", 0)
+    rc, mean_o, err_o = orc.scan_workload(w, first, count or None, n_threads=NT)
+    assert rc == 0
+    for sched in (1, 2, 3):
+        mean, err = run_gpu(w, schedule=sched, **kw)
+        assert_parity(w, mean, err, mean_o, err_o)
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 7, 8, 9, 31, 33, 255, 257])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_smallest_and_ragged_sample_counts(cfg, n):
+    """n = 2 is the smallest count the estimator accepts; the others straddle the sample-group sizes (1, 2, 4, 8) and
+    the lane counts, so groups are clipped and most lanes of the WARP / CTA schedules stay idle."""
+    scale = {1: [7], 2: [3, 5], 3: [2, 3, 2], 4: [2, 2, 3, 2], 5: [2, 2, 2, 3, 2]}[cfg]
+    _check(wl.config(cfg, scale=scale, n_samples=n))
+
+
+def test_single_point_grid_and_length_one_lists():
+    w = wl.config(5, scale=[1, 1, 1, 1, 1], n_samples=300)
+    assert w.G == 1
+    _check(w)
+    _check(wl.config(4, scale=[1, 6, 1, 5], n_samples=100))
+
+
+def test_maximum_dimensions_N16_M8():
+    """N = 16 (runtime-N kernels, 16 Philox blocks per 4-sample group) and M = 8 lists."""
+    lists = [wl.linspace(0.0, 0.3, c) for c in (2, 1, 3, 2, 1, 2, 2, 3)]
+    w = wl.Workload("p6_max", wl.P6_SIN_SUM, np.array([0.0, 1.0] * 16), lists, 203, 11, wl.PREC_F64, np.zeros(0))
+    _check(w)
+    w32 = wl.Workload("p6_max32", wl.P6_SIN_SUM, np.array([0.0, 0.5] * 16), lists, 203, 11, wl.PREC_F32E, np.zeros(0))
+    _check(w32)
+    w3 = wl.config(3, scale=[3, 2, 3], n_samples=130)
+    w3.bounds = np.array([0.0, 1.0] * 16)
+    _check(w3)
+
+
+def test_empty_ranges_enqueue_nothing():
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(2, scale=[4, 5], n_samples=10)
+    mean = torch.full((4,), -3.0, dtype=torch.float64, device="cuda")
+    err = torch.full((4,), -3.0, dtype=torch.float64, device="cuda")
+    # first_index == G with count 0 (= "to the end of the grid"): nothing to do, status OK, outputs untouched
+    tm = zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, mean, err, first_index=w.G, count=0,
+                        timing=True)
+    torch.cuda.synchronize()
+    assert torch.all(mean == -3.0) and torch.all(err == -3.0)
+    assert tm["gpu_launches"] == 0 and tm["n_batches"] == 0
+    with pytest.raises(zb.ZmcError):       # a range reaching past the grid is an argument error
+        zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, mean, err, first_index=w.G - 1, count=2)
+
+
+def test_ragged_subranges_and_batches_fp32_host_output():
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(5, scale=[3, 4, 5, 3, 7], n_samples=70)        # G = 1260
+    first, count = 13, 1009                                      # prime count, 7 batches of 150 + one of 109... ragged
+    rc, mean_o, err_o = orc.scan_workload(w, first, count, n_threads=NT)
+    for sched in (1, 2, 3):
+        m, e, tm = zb.scan_workload(w, schedule=sched, first_index=first, count=count, batch_points=150, host_out=True,
+                                    timing=True)
+        torch.cuda.synchronize()
+        assert tm["n_batches"] == 7 and tm["d2h_bytes"] == 8 * count
+        assert_parity(w, m.numpy(), e.numpy(), mean_o, err_o)
+
+
+def test_lists_too_long_for_shared_memory_staging():
+    """2 x 40 000 doubles = 640 KB of lists: the THREAD schedule falls back to reading them through L1/L2."""
+    lists = [wl.linspace(0.5, 5.0, 40_000), wl.linspace(0.5, 5.0, 40_000)]
+    w = wl.Workload("long_lists", wl.C2_SIN_XY2, np.array([0.0, wl.PI, 0.0, wl.PI]), lists, 64, 3, wl.PREC_F64, np.zeros(0))
+    first = 40_000 * 12_345 + 39_990                             # straddles a row of the grid
+    _check(w, first_index=first, count=700)
+
+
+def test_seed_uses_all_64_bits():
+    w = wl.config(1, scale=[5], n_samples=50)
+    w.seed = 0x0123456789ABCDEF
+    _check(w)
+    a, _ = run_gpu(w, schedule=1)
+    w.seed = 0x0123456789ABCDEF ^ (1 << 40)
+    b, _ = run_gpu(w, schedule=1)
+    assert not np.array_equal(a, b)
