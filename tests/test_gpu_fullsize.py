@@ -110,3 +110,46 @@ def test_cfg5_full_size_streamed_to_pinned_host():
     # D2H hidden behind compute (north_star): what is exposed is at most the last batch's copy plus launch gaps
     last_copy_ms = tm["d2h_ms"] / tm["n_batches"] * 1.5
     assert tm["exposed_d2h_ms"] <= last_copy_ms + 5.0, tm
+
+
+def _xsum_base100(count, M):
+    """sum_l x_l for flat indices 0..count-1 of the paper's grids (lists {0..99}, last list fastest)."""
+    t = np.arange(count, dtype=np.int64)
+    xsum = np.zeros(count)
+    for _ in range(M):
+        xsum += t % 100
+        t //= 100
+    return xsum
+
+
+# ---- NEXT-1: the paper's own workloads (PAPER.md:69-77 Eq. 2 / Table 1, PAPER.md:118-138 Eq. 4 / Table 2) ----------
+
+@pytest.mark.parametrize("M,N", [(1, 1), (2, 3), (3, 2), (4, 1)])
+def test_paper_table1_shapes_full_grid_sampled(M, N):
+    """Eq. (2): sin(sum y + sum x) on [0,10]^N, x_l in {0..99}, 100^M grid points, 10^4 samples, one batch."""
+    w = wl.paper_eq2(M, N)
+    mean, err, tm = gpu_scan(w)
+    assert len(mean) == w.G == 100 ** M and tm["n_batches"] == 1
+    check(w, mean, err, q17_indices(w.G, min(w.G, 20_000), 0))
+    # the paper's error metric, Eq. (3) with abs() in the denominator (reading Q14), against the closed form
+    exact = cf.p6_mean(_xsum_base100(w.G, M), N, 10.0)
+    keep = np.abs(exact) > 1e-3 * 10.0 ** N
+    z = (mean - exact) / err
+    assert np.mean(np.abs(z) <= 5) >= 0.999
+    delta_r = np.mean(np.abs(exact[keep] - mean[keep]) / np.abs(exact[keep]))
+    assert np.isfinite(delta_r)
+
+
+def test_paper_table2_batch_sampled():
+    """Eq. (4): one Table-2 batch = the first 10^6 of the 10^8 grid points x 10^5 samples (the workload bench.py
+    --workload eq4 times).  PAPER.md:130: 'the relative error at each parameter grid is always smaller 0.2'."""
+    w = wl.paper_eq4()
+    count = 10 ** 6
+    mean, err, tm = gpu_scan(w, first_index=0, count=count)
+    idx = q17_indices(count, 300, 0)
+    check(w, mean, err, idx)
+    exact = cf.p6_mean(_xsum_base100(count, 4), 6, 1.0)
+    z = (mean - exact) / err
+    assert np.mean(np.abs(z) <= 5) >= 0.999
+    big = np.abs(exact) > 0.05                       # away from the zeros of sin, where a relative error is meaningful
+    assert np.max(np.abs(mean[big] - exact[big]) / np.abs(exact[big])) < 0.2
