@@ -32,7 +32,9 @@
 #ifndef ZMC_H_
 #define ZMC_H_
 
+#ifndef __CUDACC_RTC__      /* NVRTC (user integrands) has no host headers; zmc_compat.h supplies the types */
 #include <stdint.h>
+#endif
 
 #ifdef __cplusplus
 extern "C" {
@@ -56,7 +58,8 @@ typedef enum zmc_status {
     ZMC_ERR_SHAPE_MISMATCH = 3,    /* (N, M, n_consts) not accepted by that family */
     ZMC_ERR_GRID_TOO_LARGE = 4,    /* prod(count) > 2^48, or one list longer than 2^31-1 */
     ZMC_ERR_OUT_OF_MEMORY = 5,
-    ZMC_ERR_CUDA = 6               /* see zmc_last_cuda_error() */
+    ZMC_ERR_CUDA = 6,              /* see zmc_last_cuda_error() */
+    ZMC_ERR_COMPILE = 7            /* zmc_register_integrand: NVRTC missing or the body does not compile; see zmc_last_compile_log() */
 } zmc_status;
 
 /* Integrand families g(y; x), SURVEY.md 8(c) S7 / BASELINE.json configs.  y_k is 0-based. */
@@ -125,6 +128,7 @@ typedef struct zmc_integrand_info {
     int32_t has_closed_form;
 } zmc_integrand_info;
 
+#ifndef __CUDACC_RTC__      /* the entry points are host functions: not part of what NVRTC compiles */
 /*
  * zmc_scan -- mean and standard error of the plain Monte-Carlo estimate at every grid point
  * (PAPER.md:55-65).  Defaults: fp64 path, double outputs in DEVICE memory, one batch, AUTO schedule.
@@ -158,8 +162,24 @@ ZMC_API int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N);
 /* Batch b of a range cut into batches of batch_points: writes its (first, count). Returns the number of batches. */
 ZMC_API int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_points, int64_t b,
                         uint64_t* batch_first, uint64_t* batch_count);
-/* Free the cached per-device scratch (staging buffers, streams, events). */
+/*
+ * zmc_register_integrand -- a user-defined integrand ("users have a full flexibility to define their own
+ * integrands", :49, :162; the paper JIT-compiles a Python function, here it is CUDA C++ compiled with NVRTC for
+ * sm_100a into the same kernel the built-in families use).
+ *   body   the body of   template <typename R> __device__ R g(const R* y, const R* x, const R* c)
+ *          y: the N sample coordinates y_k = a_k + (b_k - a_k) u_k, x: the M parameter values of the grid point,
+ *          c: the n_consts constants of zmc_options.consts; R is double (ZMC_PREC_F64) or float (ZMC_PREC_F32E).
+ *          Example: "return exp(-x[0] * y[0] * y[0]) * cos(x[1] * y[1] + c[0]);"
+ *   N, M, n_consts   the shape the integrand accepts (anything else is ZMC_ERR_SHAPE_MISMATCH at scan time)
+ *   integrand_id     out: an id >= 1000 to pass to zmc_scan / zmc_scan_ex (valid until zmc_shutdown)
+ * Host strings are copied.  ZMC_ERR_COMPILE: libnvrtc.so.12 not found or compilation failed (log below);
+ * ZMC_ERR_CUDA: compiled, but the code could not be loaded (no usable device).  fast_math is ignored for user integrands.
+ */
+ZMC_API zmc_status zmc_register_integrand(const char* name, const char* body, int N, int M, int n_consts, int* integrand_id);
+ZMC_API const char* zmc_last_compile_log(void);   /* NVRTC log of the last zmc_register_integrand on this thread */
+/* Free the cached per-device scratch (staging buffers, streams, events) and unload user integrands. */
 ZMC_API void zmc_shutdown(void);
+#endif /* !__CUDACC_RTC__ */
 
 #ifdef __cplusplus
 }

@@ -92,10 +92,23 @@ static double mirror(double v, int mode)
     return mode == MODE_F32_MIRROR ? (double)(float)v : v;
 }
 
+/* ---- NEXT-3: a user-defined integrand g(y; x) ("users have a full flexibility to define their
+ *      own integrands").  The test harness compiles the user's C expression with gcc and hands the function in;
+ *      any integrand id >= FAM_USER evaluates it.  Always evaluated in double (mirror mode rounds its inputs). ---- */
+#define FAM_USER 1000
+typedef double (*zmc_oracle_user_fn)(const double *y, const double *x, const double *c);
+static zmc_oracle_user_fn user_g = 0;
+static int user_N = 0, user_M = 0, user_nc = 0;
+void zmc_oracle_set_user(zmc_oracle_user_fn g, int N, int M, int n_consts)
+{
+    user_g = g; user_N = N; user_M = M; user_nc = n_consts;
+}
+
 /* ---- S7: the integrand families.  y[k] is 0-based, x[i] holds x_{i+1}. ---- */
 static double integrand(int id, int N, int M, const double *y, const double *x,
                         const double *consts)
 {
+    if (id >= FAM_USER) return user_g(y, x, consts);
     switch (id) {
     case FAM_C1:
         return cos(x[0] * y[0]);
@@ -148,6 +161,7 @@ static double integrand(int id, int N, int M, const double *y, const double *x,
 /* accepted (N, M, n_consts) per family; mirrors S7, returns 0 ok */
 static int check_shape(int id, int N, int M, int n_consts, const double *consts)
 {
+    if (id >= FAM_USER) return !user_g ? 2 : (N == user_N && M == user_M && n_consts == user_nc) ? 0 : 3;
     switch (id) {
     case FAM_C1: return (N == 1 && M == 1) ? 0 : 3;
     case FAM_C2: return (N == 2 && M == 2) ? 0 : 3;

@@ -48,6 +48,35 @@ def uniform(w: int, mode: int) -> float:
     return float(lib().zmc_oracle_uniform(w, mode))
 
 
+USER_FN = ctypes.CFUNCTYPE(ctypes.c_double, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                           ctypes.POINTER(ctypes.c_double))
+_user_keepalive = []
+
+
+def set_user_integrand(c_body: str, N: int, M: int, n_consts: int = 0):
+    """Compile `double g(const double* y, const double* x, const double* c) { <c_body> }` with gcc (R = double) and
+    make it the integrand of every id >= 1000.  The same body text is what zmc_register_integrand hands to NVRTC."""
+    import hashlib
+    import subprocess
+    import tempfile
+    src = ("#include <math.h>\n#define R double\n"
+           "double zmc_user_g(const double* y, const double* x, const double* c) {\n" + c_body + "\n}\n")
+    d = os.path.join(tempfile.gettempdir(), "zmc_oracle_user")
+    os.makedirs(d, exist_ok=True)
+    base = os.path.join(d, hashlib.sha1(src.encode()).hexdigest()[:16])
+    if not os.path.exists(base + ".so"):
+        with open(base + ".c", "w") as f:
+            f.write(src)
+        subprocess.run(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-shared", "-fPIC", base + ".c", "-o", base + ".so", "-lm"],
+                       check=True)
+    so = ctypes.CDLL(base + ".so")
+    fn = ctypes.cast(so.zmc_user_g, USER_FN)
+    _user_keepalive.append((so, fn))
+    lib().zmc_oracle_set_user.restype = None
+    lib().zmc_oracle_set_user.argtypes = [USER_FN, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+    lib().zmc_oracle_set_user(fn, N, M, n_consts)
+
+
 def _marshal(bounds, lists, consts):
     b = np.ascontiguousarray(bounds, dtype=np.float64)
     ls = [np.ascontiguousarray(l, dtype=np.float64) for l in lists]

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libzmc.so")
 # --- mirrors of include/zmc.h ----------------------------------------------------------------
 ZMC_OK, ZMC_ERR_INVALID_ARG, ZMC_ERR_UNKNOWN_INTEGRAND, ZMC_ERR_SHAPE_MISMATCH = 0, 1, 2, 3
 ZMC_ERR_GRID_TOO_LARGE, ZMC_ERR_OUT_OF_MEMORY, ZMC_ERR_CUDA = 4, 5, 6
+ZMC_ERR_COMPILE = 7
 ZMC_PREC_F64, ZMC_PREC_F32E = 0, 1
 ZMC_OUT_F64, ZMC_OUT_F32 = 0, 1
 ZMC_LOC_DEVICE, ZMC_LOC_HOST = 0, 1
@@ -27,7 +28,8 @@ ZMC_FAST_MATH_DEFAULT, ZMC_FAST_MATH_OFF, ZMC_FAST_MATH_ON = -1, 0, 1
 
 EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info_at",
            "zmc_integrand_info_by_id", "zmc_status_string", "zmc_last_cuda_error", "zmc_version",
-           "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown"]
+           "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown",
+           "zmc_register_integrand", "zmc_last_compile_log"]
 
 
 class zmc_param_list(ctypes.Structure):
@@ -103,6 +105,10 @@ def load():
                                     P(ctypes.c_uint64), P(ctypes.c_uint64)]
     lib.zmc_batch_range.restype = ctypes.c_int64
     lib.zmc_shutdown.restype = None
+    lib.zmc_register_integrand.argtypes = [ctypes.c_char_p, ctypes.c_char_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                           P(ctypes.c_int)]
+    lib.zmc_register_integrand.restype = ctypes.c_int
+    lib.zmc_last_compile_log.restype = ctypes.c_char_p
     _lib = lib
     return lib
 
@@ -241,6 +247,22 @@ def zmc_integrands():
                     "M": (info.M_min, info.M_max), "n_consts": info.n_consts,
                     "has_closed_form": bool(info.has_closed_form)})
     return out
+
+
+def zmc_register_integrand(name: str, body: str, N: int, M: int, n_consts: int = 0) -> int:
+    """Compile a user integrand (body of `template <typename R> __device__ R g(const R* y, const R* x, const R* c)`)
+    with NVRTC; returns its integrand id.  Raises ZmcError (status ZMC_ERR_COMPILE carries the NVRTC log)."""
+    lib = load()
+    out = ctypes.c_int(0)
+    st = lib.zmc_register_integrand(name.encode(), body.encode(), N, M, n_consts, ctypes.byref(out))
+    if st != ZMC_OK:
+        log = (lib.zmc_last_compile_log() or b"").decode(errors="replace")
+        raise ZmcError(st, lib.zmc_status_string(st).decode() + (": " + log[-2000:] if log else ""))
+    return int(out.value)
+
+
+def zmc_last_compile_log() -> str:
+    return (load().zmc_last_compile_log() or b"").decode(errors="replace")
 
 
 def zmc_version() -> str:

@@ -18,8 +18,26 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libzmc.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+INCLUDE = os.path.normpath(os.path.join(HERE, "..", "include"))
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-I", INCLUDE, "-I", OBJ,
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+# headers handed to NVRTC when a user integrand is compiled at run time (zmc_register_integrand): embedded as strings
+RTC_HEADERS = ["zmc_compat.h", "zmc_params.h", "zmc_math.cuh", "zmc_families.cuh", "zmc_kernel.cuh"]
+
+
+def _write_rtc_headers():
+    """build/zmc_rtc_headers.inc: {name, text} pairs of the kernel headers (+ zmc.h) as raw string literals."""
+    out = os.path.join(OBJ, "zmc_rtc_headers.inc")
+    parts = []
+    for name, path in [(h, os.path.join(CSRC, h)) for h in RTC_HEADERS] + [("zmc.h", os.path.join(INCLUDE, "zmc.h"))]:
+        text = open(path).read()
+        chunks = [text[i:i + 8000] for i in range(0, len(text), 8000)]       # stay below the literal length limit
+        parts.append('{"%s", %s},' % (name, " ".join('R"ZMCHDR(%s)ZMCHDR"' % c for c in chunks)))
+    new = "\n".join(parts) + "\n"
+    if not os.path.exists(out) or open(out).read() != new:
+        with open(out, "w") as f:
+            f.write(new)
+    return out
 
 
 def _newest(paths):
@@ -30,8 +48,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     deps = glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + \
         [os.path.join(HERE, "..", "include", "zmc.h")]
-    dep_time = _newest(deps)
     os.makedirs(OBJ, exist_ok=True)
+    deps.append(_write_rtc_headers())
+    dep_time = _newest(deps)
     jobs = []
     objs = []
     for src in srcs:
@@ -47,7 +66,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 if res.returncode:
                     raise RuntimeError("nvcc failed: " + " ".join(res.args))
     if jobs or not os.path.exists(LIB) or os.path.getmtime(LIB) < _newest(objs):
-        cmd = [NVCC, "-shared", "-o", LIB + ".tmp"] + objs
+        cmd = [NVCC, "-shared", "-o", LIB + ".tmp"] + objs + ["-ldl"]
         subprocess.run(cmd, check=True)
         os.replace(LIB + ".tmp", LIB)
     return LIB

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "zmc_params.h"
+#include "zmc_rtc.h"
 
 namespace zmc {
 extern const KernelEntry kEntriesC12[];  extern const int kNumEntriesC12;
@@ -51,9 +52,14 @@ zmc_status cuda_fail(cudaError_t e) {
         if (e__ != cudaSuccess) return cuda_fail(e__);   \
     } while (0)
 
-const zmc_integrand_info* find_family(int id) {
+// Built-in family or a registered user integrand (ids >= kFirstUserId); `storage` backs the latter's info.
+const zmc_integrand_info* find_family(int id, zmc_integrand_info* storage) {
     for (int i = 0; i < kNumFamilies; ++i)
         if (kFamilies[i].id == id) return &kFamilies[i];
+    if (const UserIntegrand* u = find_user_integrand(id)) {
+        *storage = zmc_integrand_info{u->id, u->name.c_str(), u->N, u->N, u->M, u->M, u->n_consts, 0};
+        return storage;
+    }
     return nullptr;
 }
 
@@ -110,7 +116,8 @@ zmc_status validate(int id, int N, const double* bounds, int M, const zmc_param_
     }
     for (int c = 0; c < o.n_consts; ++c)
         if (!std::isfinite(o.consts[c])) return ZMC_ERR_INVALID_ARG;
-    const zmc_integrand_info* fam = find_family(id);
+    zmc_integrand_info user_info;
+    const zmc_integrand_info* fam = find_family(id, &user_info);
     if (!fam) return ZMC_ERR_UNKNOWN_INTEGRAND;
     if (N < fam->N_min || N > fam->N_max || M < fam->M_min || M > fam->M_max || o.n_consts != fam->n_consts)
         return ZMC_ERR_SHAPE_MISMATCH;
@@ -219,7 +226,8 @@ zmc_status zmc_integrand_info_at(int index, zmc_integrand_info* info) {
 
 zmc_status zmc_integrand_info_by_id(int integrand_id, zmc_integrand_info* info) {
     if (!info) return ZMC_ERR_INVALID_ARG;
-    const zmc_integrand_info* f = find_family(integrand_id);
+    zmc_integrand_info user_info;
+    const zmc_integrand_info* f = find_family(integrand_id, &user_info);
     if (!f) return ZMC_ERR_UNKNOWN_INTEGRAND;
     *info = *f;
     return ZMC_OK;
@@ -234,6 +242,7 @@ const char* zmc_status_string(zmc_status s) {
         case ZMC_ERR_GRID_TOO_LARGE: return "parameter grid too large";
         case ZMC_ERR_OUT_OF_MEMORY: return "out of memory";
         case ZMC_ERR_CUDA: return "CUDA error (see zmc_last_cuda_error)";
+        case ZMC_ERR_COMPILE: return "user integrand did not compile (see zmc_last_compile_log)";
     }
     return "unknown status";
 }
@@ -285,6 +294,7 @@ void zmc_shutdown(void) {
         free_scratch(g_scratch[d]);
     }
     if (have) cudaSetDevice(cur);
+    unload_user_integrands();
 }
 
 zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
@@ -310,8 +320,9 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
     const bool f32e = o.precision == ZMC_PREC_F32E;
     const int fast = f32e ? (o.fast_math == ZMC_FAST_MATH_OFF ? 0 : 1) : 0;
     const int schedule = o.schedule == ZMC_SCHED_AUTO ? zmc_pick_schedule(count, n_samples, N) : o.schedule;
-    const KernelEntry* kern = find_kernel(integrand_id, N, o.precision, fast, schedule);
-    if (!kern) return ZMC_ERR_UNKNOWN_INTEGRAND;
+    const UserIntegrand* user = integrand_id >= kFirstUserId ? find_user_integrand(integrand_id) : nullptr;
+    const KernelEntry* kern = user ? nullptr : find_kernel(integrand_id, N, o.precision, fast, schedule);
+    if (!kern && !user) return ZMC_ERR_UNKNOWN_INTEGRAND;
     if (timing) timing->schedule = schedule;
     if (count == 0) return ZMC_OK;
 
@@ -448,7 +459,8 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
                 p.base_digits[0] = (uint32_t)rest;
             }
             const uint64_t grid = (lc + per_cta - 1) / per_cta;
-            ZMC_CUDA(kern->launch(p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
+            if (user) ZMC_CUDA(launch_user(*user, o.precision, schedule, p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
+            else ZMC_CUDA(kern->launch(p, dst_mean, dst_err, (int)grid, smem_bytes, stream));
             ++launches;
             lc_done = lc;
         }

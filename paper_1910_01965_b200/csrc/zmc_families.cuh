@@ -9,7 +9,7 @@
 //                          real eval_shifted(const uint32_t* w, real K) const; // g - K; w: the N words of one sample
 //                          real eval(const uint32_t* w) const; }               // g (used once per point, for K)
 #pragma once
-#include <type_traits>
+#include "zmc_compat.h"
 #include "zmc_math.cuh"
 #include "zmc_params.h"
 

@@ -200,6 +200,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     }
 }
 
+#ifndef __CUDACC_RTC__
 template <class Fam, int SCHED>
 cudaError_t launch_scan(const ScanParams& p, void* out_mean, void* out_stderr, int grid, size_t smem_bytes,
                         cudaStream_t stream)
@@ -234,5 +235,7 @@ cudaError_t launch_scan(const ScanParams& p, void* out_mean, void* out_stderr, i
 #define ZMC_ENTRY_DIAG(FAMILY_ID, F)                                         \
     ZMC_ENTRY(FAMILY_ID, 0, ZMC_PREC_F64, 0, F<double>),                     \
     ZMC_ENTRY(FAMILY_ID, 0, ZMC_PREC_F32E, 0, F<float>)
+
+#endif  // !__CUDACC_RTC__
 
 }  // namespace zmc

@@ -7,8 +7,7 @@
 // odd polynomial with immediate coefficients -- no table loads, no slow path) and thin wrappers
 // over the MUFU transcendentals for the fp32 path.
 #pragma once
-#include <cstdint>
-#include <cuda_runtime.h>
+#include "zmc_compat.h"
 
 #ifndef ZMC_F64_UNIT_I2F
 #define ZMC_F64_UNIT_I2F 0

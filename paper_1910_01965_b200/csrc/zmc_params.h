@@ -1,8 +1,7 @@
 // zmc_params.h -- the kernel argument block (host fills it, kernels read it from the constant bank).
 #pragma once
-#include <cstdint>
-#include <cuda_runtime.h>
-#include "../../include/zmc.h"
+#include "zmc_compat.h"
+#include "zmc.h"
 
 namespace zmc {
 
@@ -30,6 +29,7 @@ enum { kSchedThread = ZMC_SCHED_THREAD, kSchedWarp = ZMC_SCHED_WARP, kSchedCta =
 
 constexpr int kThreads = 256;      // CTA size of every schedule
 
+#ifndef __CUDACC_RTC__
 // launcher signature shared by the dispatch table (zmc_api.cu) and the instantiation units
 typedef cudaError_t (*LaunchFn)(const ScanParams& p, void* out_mean, void* out_stderr, int grid,
                                 size_t smem_bytes, cudaStream_t stream);
@@ -39,5 +39,6 @@ struct KernelEntry {
     LaunchFn launch;
     const void* func;              // for occupancy queries / attributes
 };
+#endif  // !__CUDACC_RTC__
 
 }  // namespace zmc

@@ -1,0 +1,23 @@
+// zmc_rtc.h -- internal interface between zmc_api.cu and zmc_rtc.cu (user integrands compiled with NVRTC).
+#pragma once
+#include <string>
+#include "zmc_params.h"
+
+namespace zmc {
+
+constexpr int kFirstUserId = 1000;
+
+struct UserIntegrand {
+    int id = 0;
+    std::string name;
+    int N = 0, M = 0, n_consts = 0;
+    cudaLibrary_t lib = nullptr;
+    cudaKernel_t kern[2][3] = {};        // [precision][schedule - 1]
+};
+
+const UserIntegrand* find_user_integrand(int id);
+cudaError_t launch_user(const UserIntegrand& u, int precision, int schedule, const ScanParams& p, void* out_mean,
+                        void* out_stderr, int grid, size_t smem_bytes, cudaStream_t stream);
+void unload_user_integrands();
+
+}  // namespace zmc

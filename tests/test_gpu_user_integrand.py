@@ -1,0 +1,75 @@
+"""-m gpu: NEXT-3, user-defined integrands compiled with NVRTC, against the CPU oracle evaluating the SAME body text
+(compiled with gcc, R = double) on the same sample stream -- same tolerances as the built-in families."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import zmc_oracle as orc
+from paper_1910_01965_b200 import workloads as wl
+from test_gpu_parity import assert_parity, run_gpu
+
+pytestmark = pytest.mark.gpu
+NT = min(16, os.cpu_count() or 1)
+
+CASES = {
+    # name: (body, bounds, lists, consts, n)
+    "damped_cos": ("return exp(-x[0] * y[0] * y[0]) * cos(x[1] * y[1] + c[0]);",
+                   [0.0, 1.0, 0.0, 2.0], [wl.linspace(0.2, 3.0, 13), wl.linspace(0.5, 4.0, 11)], [0.3], 1003),
+    "rational_3d": ("R d = (R)1 + x[0] * (y[0] * y[0] + y[1] * y[1] + y[2] * y[2]); return y[0] * y[1] / (d * d) + x[1];",
+                    [-1.0, 1.0, 0.0, 2.0, 0.5, 1.5], [wl.linspace(0.1, 2.0, 7), wl.linspace(-1.0, 1.0, 5)], [], 517),
+    "sum_11d": ("R s = x[0]; for (int k = 0; k < 11; ++k) s += y[k] * (R)(k + 1); return sin(s) * c[1] + c[0];",
+                [0.0, 0.25] * 11, [wl.linspace(0.0, 3.0, 9)], [0.5, 2.0], 259),
+}
+
+
+def _workload(name, uid, precision):
+    body, bounds, lists, consts, n = CASES[name]
+    return wl.Workload(name, uid, np.array(bounds), [np.asarray(l, dtype=np.float64) for l in lists], n, 21, precision,
+                       np.array(consts, dtype=np.float64))
+
+
+@pytest.mark.parametrize("precision", [wl.PREC_F64, wl.PREC_F32E])
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_user_integrand_parity_all_schedules(name, precision):
+    from paper_1910_01965_b200 import binding as zb
+    body, bounds, lists, consts, n = CASES[name]
+    uid = zb.zmc_register_integrand(name, body, len(bounds) // 2, len(lists), len(consts))
+    assert uid >= 1000
+    orc.set_user_integrand(body, len(bounds) // 2, len(lists), len(consts))
+    w = _workload(name, uid, precision)
+    rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
+    assert rc == 0
+    for sched in (1, 2, 3):
+        mean, err = run_gpu(w, schedule=sched)
+        assert_parity(w, mean, err, mean_o, err_o)
+    # batch / sub-range invariance holds for user integrands too (same kernel template): bit-exact
+    full, _ = run_gpu(w, schedule=1)
+    part, _ = run_gpu(w, schedule=1, first_index=3, count=w.G - 5, batch_points=7)
+    assert np.array_equal(part, full[3:w.G - 2])
+
+
+def test_user_copy_of_a_builtin_family_matches_it():
+    """The user body of cfg 2's integrand goes through the generic (unfolded) evaluation; the built-in family folds the
+    affine map and uses its own sinpi: both must agree with the oracle, hence with each other, to the fp64 tolerance."""
+    from paper_1910_01965_b200 import binding as zb
+    uid = zb.zmc_register_integrand("c2_copy", "return sin(x[0] * y[0] + x[1] * y[1]);", 2, 2, 0)
+    w = wl.config(2, scale=[19, 23], n_samples=2001)
+    builtin, berr = run_gpu(w, schedule=2)
+    w.integrand_id = uid
+    user, uerr = run_gpu(w, schedule=2)
+    assert np.all(np.abs(user - builtin) <= 1e-10 * np.maximum(np.abs(builtin), berr))
+    assert np.all(np.abs(uerr - berr) <= 1e-10 * berr)
+
+
+def test_user_shape_mismatch_and_unknown_id():
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    uid = zb.zmc_register_integrand("one_d", "return y[0] * x[0];", 1, 1, 0)
+    m = torch.zeros(4, dtype=torch.float64, device="cuda")
+    with pytest.raises(zb.ZmcError) as ei:         # registered for N = 1, called with N = 2
+        zb.zmc_scan_ex(uid, [0.0, 1.0, 0.0, 1.0], [np.arange(4.0)], 10, 1, m, m.clone())
+    assert ei.value.status == zb.ZMC_ERR_SHAPE_MISMATCH
+    with pytest.raises(zb.ZmcError) as ei:
+        zb.zmc_scan_ex(uid + 500, [0.0, 1.0], [np.arange(4.0)], 10, 1, m, m.clone())
+    assert ei.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
