@@ -51,7 +51,10 @@ ALG_OPS = {
 # Workloads that scan only part of their grid per step: the paper's Table 2 batch is 10^6 of the
 # 10^8 grid points x 10^5 samples; its V100 "GPU evaluation time per batch" 18.19497 s = 5.50e9 evals/s is the one
 # published number for exactly this workload, hence the one non-null vs_baseline.
+ALG_OPS["cfg2_user"] = ALG_OPS["cfg2"]     # same method, same minimum; the generic user path executes more
 SCAN_POINTS = {"eq4": 10**6}
+# NEXT-3: the cfg2 inputs with the integrand handed over as a user body and compiled with NVRTC at run time
+USER_BODIES = {"cfg2_user": ("cfg2", "return sin(x[0] * y[0] + x[1] * y[1]);")}
 PUBLISHED_EVALS_PER_S = {"eq4": 1e6 * 1e5 / 18.19497}
 
 
@@ -67,7 +70,9 @@ PEAK_GLANE = SM_COUNT * LANES_PER_SM_CLK * SM_MAX_MHZ * 1e6 / 1e9      # 37 225 
 
 
 def build_workload(name: str, world: int):
-    w = wl.paper_eq4() if name == "eq4" else wl.config(int(name[3:]))
+    base = USER_BODIES[name][0] if name in USER_BODIES else name
+    w = wl.paper_eq4() if base == "eq4" else wl.config(int(base[3:]))
+    w.name = name
     if world > 1:       # weak scaling: N-fold longer first list, one contiguous shard per rank
         lo, hi = float(w.lists[0][0]), float(w.lists[0][-1])
         w.lists[0] = wl.linspace(lo, hi, len(w.lists[0]) * world)
@@ -113,6 +118,9 @@ class ClockSampler:
 def cpu_oracle_rate(w, seconds: float = 1.5):
     """The oracle as it stands on all host cores, on a bounded contiguous slice from the middle of the grid."""
     from oracle import zmc_oracle as orc
+    if w.name in USER_BODIES:
+        orc.set_user_integrand(USER_BODIES[w.name][1], w.N, w.M, len(w.consts))
+        w.integrand_id = max(w.integrand_id, 1000)
     cores = os.cpu_count() or 1
     first = (w.G // 2 // 1000) * 1000
     probe = max(cores * 4, min(w.G - first, max(cores * 4, int(2e6 // w.n_samples))))
@@ -183,6 +191,8 @@ def main():
     zb.load()
 
     w = build_workload(args.workload, world)
+    if w.name in USER_BODIES:
+        w.integrand_id = zb.zmc_register_integrand(w.name, USER_BODIES[w.name][1], w.N, w.M, len(w.consts))
     G_scan = SCAN_POINTS.get(w.name, w.G) * (world if w.name in SCAN_POINTS else 1)
     first, count = wl.shard_range(G_scan, rank, world)
     stream = torch.cuda.current_stream()
