@@ -49,6 +49,7 @@ extern "C" {
 #define ZMC_MAX_N 16        /* integration dimensions */
 #define ZMC_MAX_M 8         /* parameters */
 #define ZMC_MAX_CONSTS 8    /* family constants */
+#define ZMC_MAX_FARM_DEVICES 16   /* devices of one node in zmc_scan_farm */
 
 typedef enum zmc_status {
     ZMC_OK = 0,
@@ -119,6 +120,17 @@ typedef struct zmc_timing {
     int32_t reserved;
 } zmc_timing;
 
+/* What zmc_scan_farm did (the paper's allocation / evaluation view of Table 2). Host wall clock. */
+typedef struct zmc_farm_timing {
+    double wall_ms;                                  /* whole call */
+    int64_t n_batches;
+    uint64_t batch_points;
+    int32_t n_devices;
+    int32_t reserved;
+    int64_t batches_done[ZMC_MAX_FARM_DEVICES];      /* batches each device slot ended up taking (dynamic assignment) */
+    double busy_ms[ZMC_MAX_FARM_DEVICES];            /* first pull to last completion, per device slot */
+} zmc_farm_timing;
+
 typedef struct zmc_integrand_info {
     int32_t id;
     const char* name;
@@ -162,6 +174,19 @@ ZMC_API int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N);
 /* Batch b of a range cut into batches of batch_points: writes its (first, count). Returns the number of batches. */
 ZMC_API int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_points, int64_t b,
                         uint64_t* batch_first, uint64_t* batch_count);
+/*
+ * zmc_scan_farm -- the same scan farmed over several GPUs of one node ("Each batch is fed into one GPU
+ * device", :81, Table 2 :132-140).  The flat range is cut into batches of opt->batch_points (0 = about 8 per device);
+ * one host thread per entry of `devices` pulls batches from a shared counter and scans them on its device into
+ * out_mean / out_stderr, which must be HOST memory (pinned recommended; opt->out_location is ignored) of the scanned
+ * range's length.  SYNCHRONOUS: returns when every batch has landed.  No inter-device traffic; results are
+ * bit-identical to a one-device zmc_scan_ex with the same schedule, whichever device takes which batch.
+ * A device may be listed more than once (two feeder threads on one GPU).  timing may be NULL.
+ */
+ZMC_API zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                         uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, const int* devices,
+                         int n_devices, const zmc_options* opt, zmc_farm_timing* timing);
+
 /*
  * zmc_register_integrand -- a user-defined integrand ("users have a full flexibility to define their own
  * integrands", :49, :162; the paper JIT-compiles a Python function, here it is CUDA C++ compiled with NVRTC for

@@ -29,7 +29,7 @@ ZMC_FAST_MATH_DEFAULT, ZMC_FAST_MATH_OFF, ZMC_FAST_MATH_ON = -1, 0, 1
 EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info_at",
            "zmc_integrand_info_by_id", "zmc_status_string", "zmc_last_cuda_error", "zmc_version",
            "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown",
-           "zmc_register_integrand", "zmc_last_compile_log"]
+           "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm"]
 
 
 class zmc_param_list(ctypes.Structure):
@@ -52,6 +52,15 @@ class zmc_timing(ctypes.Structure):
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_ if f != "reserved"}
+
+
+ZMC_MAX_FARM_DEVICES = 16
+
+
+class zmc_farm_timing(ctypes.Structure):
+    _fields_ = [("wall_ms", ctypes.c_double), ("n_batches", ctypes.c_int64), ("batch_points", ctypes.c_uint64),
+                ("n_devices", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("batches_done", ctypes.c_int64 * ZMC_MAX_FARM_DEVICES), ("busy_ms", ctypes.c_double * ZMC_MAX_FARM_DEVICES)]
 
 
 class zmc_integrand_info(ctypes.Structure):
@@ -109,6 +118,8 @@ def load():
                                            P(ctypes.c_int)]
     lib.zmc_register_integrand.restype = ctypes.c_int
     lib.zmc_last_compile_log.restype = ctypes.c_char_p
+    lib.zmc_scan_farm.argtypes = scan_args[:9] + [P(ctypes.c_int), ctypes.c_int, P(zmc_options), P(zmc_farm_timing)]
+    lib.zmc_scan_farm.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -247,6 +258,26 @@ def zmc_integrands():
                     "M": (info.M_min, info.M_max), "n_consts": info.n_consts,
                     "has_closed_form": bool(info.has_closed_form)})
     return out
+
+
+def zmc_scan_farm(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, devices, *,
+                  precision: int = ZMC_PREC_F64, schedule: int = ZMC_SCHED_AUTO, fast_math: int = ZMC_FAST_MATH_DEFAULT,
+                  batch_points: int = 0, first_index: int = 0, count: int = 0, consts=None) -> dict:
+    """zmc_scan over several GPUs of one node (host outputs, synchronous).  Returns the farm timing as a dict."""
+    lib = load()
+    m = _Marshalled(bounds, lists, consts)
+    pm, dt_m, loc_m = _tensor_ptr(out_mean)
+    pe, dt_e, loc_e = _tensor_ptr(out_stderr)
+    if dt_m != dt_e or loc_m != ZMC_LOC_HOST or loc_e != ZMC_LOC_HOST:
+        raise ValueError("zmc_scan_farm needs two host arrays of the same dtype")
+    o = _make_options(m, precision, dt_m, ZMC_LOC_HOST, schedule, fast_math, batch_points, first_index, count)
+    devs = (ctypes.c_int * len(devices))(*devices)
+    tm = zmc_farm_timing()
+    _check(lib.zmc_scan_farm(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_samples, seed, ctypes.c_void_p(pm),
+                             ctypes.c_void_p(pe), devs, len(devices), ctypes.byref(o), ctypes.byref(tm)))
+    n = tm.n_devices
+    return {"wall_ms": tm.wall_ms, "n_batches": tm.n_batches, "batch_points": tm.batch_points, "n_devices": n,
+            "batches_done": list(tm.batches_done[:n]), "busy_ms": list(tm.busy_ms[:n])}
 
 
 def zmc_register_integrand(name: str, body: str, N: int, M: int, n_consts: int = 0) -> int:

@@ -155,10 +155,11 @@ struct DeviceScratch {
     cudaEvent_t stage_free[2] = {nullptr, nullptr};   // last copy out of stage[i]
     bool stage_used[2] = {false, false};
     cudaEvent_t kernel_done[2] = {nullptr, nullptr};
+    unsigned stage_rot = 0;                  // staging buffers alternate across batches AND across calls
 };
 constexpr int kMaxDevices = 64;
 DeviceScratch g_scratch[kMaxDevices];
-std::mutex g_mutex;
+std::mutex g_dev_mutex[kMaxDevices];     // one per device: calls on different GPUs (zmc_scan_farm) do not serialise
 
 zmc_status get_scratch(int dev, DeviceScratch** out) {
     if (dev < 0 || dev >= kMaxDevices) return ZMC_ERR_CUDA;
@@ -285,10 +286,10 @@ int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_poi
 }
 
 void zmc_shutdown(void) {
-    std::lock_guard<std::mutex> lock(g_mutex);
     int cur = 0;
     const bool have = cudaGetDevice(&cur) == cudaSuccess;
     for (int d = 0; d < kMaxDevices; ++d) {
+        std::lock_guard<std::mutex> lock(g_dev_mutex[d]);
         if (!g_scratch[d].init) continue;
         if (have) cudaSetDevice(d);
         free_scratch(g_scratch[d]);
@@ -326,9 +327,10 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
     if (timing) timing->schedule = schedule;
     if (count == 0) return ZMC_OK;
 
-    std::lock_guard<std::mutex> lock(g_mutex);
     int dev = 0;
     ZMC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return ZMC_ERR_CUDA;
+    std::lock_guard<std::mutex> lock(g_dev_mutex[dev]);
     DeviceScratch* s = nullptr;
     st = get_scratch(dev, &s);
     if (st != ZMC_OK) return st;
@@ -416,7 +418,7 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
             ZMC_CUDA(cudaMalloc(&s->stage[0], need));
             s->stage_cap = need;
         }
-        if (n_batches > 1 && !s->stage[1]) ZMC_CUDA(cudaMalloc(&s->stage[1], s->stage_cap));
+        if (!s->stage[1]) ZMC_CUDA(cudaMalloc(&s->stage[1], s->stage_cap));   // both: the buffers alternate across calls too
     }
 
     // One worker (thread / warp / CTA) per grid point, one CTA per `per_cta` points: the hardware CTA scheduler
@@ -433,7 +435,7 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
         zmc_batch_range(first, count, o.batch_points, b, &bf, &bc);
         void *dst_mean, *dst_err;
         uint64_t out_base;                     // flat index of element 0 of dst_mean / dst_err
-        const int buf = (int)(b & 1);
+        const int buf = host_out ? (int)(s->stage_rot++ & 1u) : 0;
         if (host_out) {
             if (s->stage_used[buf]) ZMC_CUDA(cudaStreamWaitEvent(stream, s->stage_free[buf], 0));
             dst_mean = s->stage[buf];
@@ -483,7 +485,7 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
     ZMC_CUDA(cudaEventRecord(slot.done, stream));
     slot.used = true;
     if (host_out) {   // join the side stream back into `stream`
-        const int last = (int)((n_batches - 1) & 1);
+        const int last = (int)((s->stage_rot - 1u) & 1u);
         ZMC_CUDA(cudaStreamWaitEvent(stream, s->stage_free[last], 0));
     }
 
