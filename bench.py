@@ -169,6 +169,7 @@ def main():
     ap.add_argument("--schedule", type=int, default=0, help="0 auto, 1 thread, 2 warp, 3 cta")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--farm-devices", default="", help="e.g. 0,1,2,3: also time zmc_scan_farm over these devices (N=1 only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "zmc" else args.warmup
 
@@ -277,6 +278,19 @@ def main():
                "d2h_gbs": float(np.mean([i["d2h_bytes"] / max(i["d2h_ms"], 1e-9) * 1e-6 for i in e_infos]))}
         launches += int(sum(i["gpu_launches"] for i in e_infos))
 
+    # ---- NEXT-2: the single-node batch farm over --farm-devices (host outputs, synchronous, host wall clock) -------
+    farm = None
+    if args.farm_devices and world == 1 and not args.no_e2e:
+        devs = [int(d) for d in args.farm_devices.split(",")]
+        f_ms = []
+        for _ in range(3):
+            tmf = zb.zmc_scan_farm(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, devs,
+                                   precision=w.precision, schedule=args.schedule, first_index=first, count=count,
+                                   batch_points=w.batch_points, consts=w.consts)
+            f_ms.append(tmf["wall_ms"])
+        farm = {"devices": devs, "value": evals_all / (min(f_ms[1:]) * 1e-3), "unit": UNIT, "wall_ms": min(f_ms[1:]),
+                "n_batches": tmf["n_batches"], "batches_done": tmf["batches_done"], "busy_ms": tmf["busy_ms"]}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -297,6 +311,7 @@ def main():
         "kernel_ms_per_step": kernel_ms,
         "clocks": clocks,
         "e2e": e2e,
+        "farm": farm,
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
                      "frac": achieved / PEAK_GLANE, "traffic": None,
