@@ -175,6 +175,22 @@ ZMC_API int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N);
 ZMC_API int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_points, int64_t b,
                         uint64_t* batch_first, uint64_t* batch_count);
 /*
+ * zmc_scan_adaptive -- per-point adaptive sample count (the paper asks the user to "determine the number
+ * of sample points based on the desired accuracy ... increase this value" by hand).  Every grid point is sampled up to
+ * the checkpoints n_first, 2 n_first, 4 n_first, ... (clipped to n_max) and stops at the first one whose standard
+ * error is <= target_stderr.  Because the sample stream is keyed by (seed, global index, word index), the estimate at
+ * a checkpoint uses exactly the first n samples: the outputs equal zmc_scan_ex(n_samples = out_n[point],
+ * schedule = ZMC_SCHED_WARP) bit for bit.
+ *   n_first   first checkpoint, a multiple of 256 (>= 256)      n_max  last checkpoint, a multiple of 8, >= n_first
+ *   out_n     samples used per point (uint32, DEVICE memory, indexed like out_mean)
+ * Outputs must be DEVICE memory (opt->out_location); opt->schedule is ignored (one warp per point); batching, sub-ranges,
+ * precision, out_dtype and timing behave as in zmc_scan_ex.
+ */
+ZMC_API zmc_status zmc_scan_adaptive(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                             uint64_t n_first, uint64_t n_max, double target_stderr, uint64_t seed, void* out_mean,
+                             void* out_stderr, uint32_t* out_n, void* stream, const zmc_options* opt, zmc_timing* timing);
+
+/*
  * zmc_scan_farm -- the same scan farmed over several GPUs of one node ("Each batch is fed into one GPU
  * device", :81, Table 2 :132-140).  The flat range is cut into batches of opt->batch_points (0 = about 8 per device);
  * one host thread per entry of `devices` pulls batches from a shared counter and scans them on its device into

@@ -29,7 +29,7 @@ ZMC_FAST_MATH_DEFAULT, ZMC_FAST_MATH_OFF, ZMC_FAST_MATH_ON = -1, 0, 1
 EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info_at",
            "zmc_integrand_info_by_id", "zmc_status_string", "zmc_last_cuda_error", "zmc_version",
            "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown",
-           "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm"]
+           "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm", "zmc_scan_adaptive"]
 
 
 class zmc_param_list(ctypes.Structure):
@@ -120,6 +120,10 @@ def load():
     lib.zmc_last_compile_log.restype = ctypes.c_char_p
     lib.zmc_scan_farm.argtypes = scan_args[:9] + [P(ctypes.c_int), ctypes.c_int, P(zmc_options), P(zmc_farm_timing)]
     lib.zmc_scan_farm.restype = ctypes.c_int
+    lib.zmc_scan_adaptive.argtypes = scan_args[:5] + [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_double, ctypes.c_uint64,
+                                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                                      P(zmc_options), P(zmc_timing)]
+    lib.zmc_scan_adaptive.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -258,6 +262,25 @@ def zmc_integrands():
                     "M": (info.M_min, info.M_max), "n_consts": info.n_consts,
                     "has_closed_form": bool(info.has_closed_form)})
     return out
+
+
+def zmc_scan_adaptive(integrand_id: int, bounds, lists, n_first: int, n_max: int, target_stderr: float, seed: int,
+                      out_mean, out_stderr, out_n, stream=None, *, precision: int = ZMC_PREC_F64,
+                      fast_math: int = ZMC_FAST_MATH_DEFAULT, batch_points: int = 0, first_index: int = 0,
+                      count: int = 0, consts=None, timing: bool = False) -> Optional[dict]:
+    """include/zmc.h zmc_scan_adaptive.  out_n: int32/uint32 torch CUDA tensor (samples used per point)."""
+    m = _Marshalled(bounds, lists, consts)
+    pm, dm, lm = _tensor_ptr(out_mean)
+    pe, de, le = _tensor_ptr(out_stderr)
+    if (dm, lm) != (de, le) or not out_n.is_cuda or out_n.element_size() != 4:
+        raise ZmcError(ZMC_ERR_INVALID_ARG, "outputs must share dtype/location; out_n must be a 4-byte CUDA tensor")
+    o = _make_options(m, precision, dm, lm, ZMC_SCHED_AUTO, fast_math, batch_points, first_index, count)
+    tm = zmc_timing() if timing else None
+    _check(load().zmc_scan_adaptive(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_first, n_max, target_stderr, seed,
+                                    ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(out_n.data_ptr()),
+                                    ctypes.c_void_p(_stream_handle(stream)), ctypes.byref(o),
+                                    ctypes.byref(tm) if timing else None))
+    return tm.as_dict() if timing else None
 
 
 def zmc_scan_farm(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, devices, *,

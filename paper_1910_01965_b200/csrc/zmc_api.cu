@@ -304,13 +304,23 @@ zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M, const 
                        nullptr, nullptr);
 }
 
-zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
-                       uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream_v,
-                       const zmc_options* opt, zmc_timing* timing) {
+// adaptive scan (NEXT-4): n_samples is the first checkpoint; these are the other arguments of zmc_scan_adaptive
+struct AdaptArgs { uint64_t n_max; double target; uint32_t* out_n; };
+
+static zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                            uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream_v,
+                            const zmc_options* opt, zmc_timing* timing, const AdaptArgs* ad) {
     // ---- H1: validate -----------------------------------------------------------------------
     Options o;
     zmc_status st = read_options(opt, &o);
     if (st != ZMC_OK) return st;
+    if (ad) {
+        if (!ad->out_n || o.out_location != ZMC_LOC_DEVICE) return ZMC_ERR_INVALID_ARG;     // device outputs only
+        if (n_samples < 256 || n_samples % 256 != 0) return ZMC_ERR_INVALID_ARG;           // lane ownership, see kernel
+        if (ad->n_max < n_samples || ad->n_max % 8 != 0 || ad->n_max > 0xFFFFFFF8ull) return ZMC_ERR_INVALID_ARG;
+        if (ad->n_max * (uint64_t)(N > 0 ? N : 1) > (1ull << 34)) return ZMC_ERR_INVALID_ARG;
+        if (!(ad->target >= 0.0) || !std::isfinite(ad->target)) return ZMC_ERR_INVALID_ARG;
+    }
     uint64_t G = 0, first = 0, count = 0;
     st = validate(integrand_id, N, bounds, M, lists, n_samples, o, &G, &first, &count);
     if (st != ZMC_OK) return st;
@@ -320,11 +330,12 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
 
     const bool f32e = o.precision == ZMC_PREC_F32E;
     const int fast = f32e ? (o.fast_math == ZMC_FAST_MATH_OFF ? 0 : 1) : 0;
-    const int schedule = o.schedule == ZMC_SCHED_AUTO ? zmc_pick_schedule(count, n_samples, N) : o.schedule;
+    const int schedule = ad ? (int)kSchedAdapt
+                       : o.schedule == ZMC_SCHED_AUTO ? zmc_pick_schedule(count, n_samples, N) : o.schedule;
     const UserIntegrand* user = integrand_id >= kFirstUserId ? find_user_integrand(integrand_id) : nullptr;
     const KernelEntry* kern = user ? nullptr : find_kernel(integrand_id, N, o.precision, fast, schedule);
     if (!kern && !user) return ZMC_ERR_UNKNOWN_INTEGRAND;
-    if (timing) timing->schedule = schedule;
+    if (timing) timing->schedule = ad ? (int)ZMC_SCHED_WARP : schedule;
     if (count == 0) return ZMC_OK;
 
     int dev = 0;
@@ -424,7 +435,9 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
     // One worker (thread / warp / CTA) per grid point, one CTA per `per_cta` points: the hardware CTA scheduler
     // balances the load.  A batch larger than kMaxLaunchPoints is cut into several launches so that local point
     // indices and the grid size stay 32-bit.
-    const uint64_t per_cta = schedule == ZMC_SCHED_THREAD ? kThreads : schedule == ZMC_SCHED_WARP ? kThreads / 32 : 1;
+    const uint64_t per_cta = schedule == ZMC_SCHED_THREAD ? kThreads
+                           : (schedule == ZMC_SCHED_WARP || schedule == kSchedAdapt) ? kThreads / 32 : 1;
+    if (ad) { p.n_max = (uint32_t)ad->n_max; p.target = ad->target; p.out_n = ad->out_n; }
     constexpr uint64_t kMaxLaunchPoints = 1ull << 30;
 
     std::vector<TimedSpan> t_kernel, t_copy;
@@ -505,6 +518,19 @@ zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, con
         timing->h2d_bytes = total * sizeof(double);
     }
     return ZMC_OK;
+}
+
+zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                       uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream,
+                       const zmc_options* opt, zmc_timing* timing) {
+    return scan_impl(integrand_id, N, bounds, M, lists, n_samples, seed, out_mean, out_stderr, stream, opt, timing, nullptr);
+}
+
+zmc_status zmc_scan_adaptive(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                             uint64_t n_first, uint64_t n_max, double target_stderr, uint64_t seed, void* out_mean,
+                             void* out_stderr, uint32_t* out_n, void* stream, const zmc_options* opt, zmc_timing* timing) {
+    const AdaptArgs ad{n_max, target_stderr, out_n};
+    return scan_impl(integrand_id, N, bounds, M, lists, n_first, seed, out_mean, out_stderr, stream, opt, timing, &ad);
 }
 
 }  // extern "C"

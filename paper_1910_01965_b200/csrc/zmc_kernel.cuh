@@ -42,6 +42,31 @@ template <typename R> struct Accum {
     }
 };
 
+// H3: mixed-radix decode.  digits(t) = digits(first) + digits(local) with carries: the 64-bit part was done on the
+// host, the per-point part is 32-bit division only.  Writes the point's M parameter values (evaluation type) to x.
+template <typename R>
+__device__ __forceinline__ void decode_point(const ScanParams& p, uint32_t local, const R* __restrict__ slist, R (&x)[ZMC_MAX_M]) {
+    const int M = (int)p.n_par;
+    uint32_t rest = local, carry = 0;
+#pragma unroll
+    for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
+        if (i < M) {
+            const uint32_t L = p.counts[i];
+            const uint32_t q = rest / L;
+            uint32_t d = p.base_digits[i] + (rest - q * L) + carry;
+            carry = d >= L ? 1u : 0u;
+            d -= carry ? L : 0u;
+            rest = q;
+            const uint32_t idx = p.list_off[i] + d;
+            x[i] = p.stage_smem ? slist[idx] : (R)__ldg(p.lists + idx);
+        } else {
+            x[i] = (R)0;
+        }
+    }
+    const uint32_t idx0 = p.list_off[0] + p.base_digits[0] + rest + carry;
+    x[0] = p.stage_smem ? slist[idx0] : (R)__ldg(p.lists + idx0);
+}
+
 template <class Fam, int SCHED>
 __global__ void __launch_bounds__(kThreads, std::is_same<typename Fam::real, double>::value ? 3 : 4)
 zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mean, void* __restrict__ out_stderr)
@@ -52,7 +77,6 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     constexpr int S = GS::S;
     const int N = kN ? kN : (int)p.n_dim;
     const int NB = kN ? GS::NB : N;
-    const int M = (int)p.n_par;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     R* slist = reinterpret_cast<R*>(smem_raw);
@@ -74,29 +98,8 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     if (local >= p.count) return;                   // uniform per warp (WARP) / per CTA (CTA)
     const uint32_t t_lo = (uint32_t)p.first + local;      // no carry: a launch never straddles a multiple of 2^32
 
-    // H3: mixed-radix decode.  digits(t) = digits(first) + digits(local) with carries: the 64-bit part was done on
-    // the host, the per-point part is 32-bit division only.
     R x[ZMC_MAX_M];
-    {
-        uint32_t rest = local, carry = 0;
-#pragma unroll
-        for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
-            if (i < M) {
-                const uint32_t L = p.counts[i];
-                const uint32_t q = rest / L;
-                uint32_t d = p.base_digits[i] + (rest - q * L) + carry;
-                carry = d >= L ? 1u : 0u;
-                d -= carry ? L : 0u;
-                rest = q;
-                const uint32_t idx = p.list_off[i] + d;
-                x[i] = p.stage_smem ? slist[idx] : (R)__ldg(p.lists + idx);
-            } else {
-                x[i] = (R)0;
-            }
-        }
-        const uint32_t idx0 = p.list_off[0] + p.base_digits[0] + rest + carry;
-        x[0] = p.stage_smem ? slist[idx0] : (R)__ldg(p.lists + idx0);
-    }
+    decode_point<R>(p, local, slist, x);
 
     const uint32_t n = p.n;
     const uint32_t n_full = n / S;                 // full groups; the last group may be clipped
@@ -200,6 +203,91 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     }
 }
 
+// NEXT-4: per-point adaptive sample count.  PAPER.md:116 leaves it to the user to "determine the
+// number of sample points based on the desired accuracy ... increase this value"; here the kernel does it: one warp per
+// grid point samples up to the checkpoints n_0 = p.n, 2 n_0, 4 n_0, ... (clipped to p.n_max) and stops at the first
+// one where stderr <= p.target.  The stream is keyed by (seed, t, word index), so the estimate at a checkpoint uses
+// exactly the first n words (prefix property) and -- n_0 being a multiple of 256, hence every checkpoint a multiple
+// of 32 groups -- lane l owns groups l, l+32, ... exactly as in the fixed-n WARP schedule: the result is bit-identical
+// to zmc_scan_ex(n_samples = n_used, schedule = WARP).
+template <class Fam>
+__global__ void __launch_bounds__(kThreads, std::is_same<typename Fam::real, double>::value ? 3 : 4)
+zmc_adapt_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mean, void* __restrict__ out_stderr)
+{
+    using R = typename Fam::real;
+    constexpr int kN = Fam::kN;
+    using GS = GroupShape<kN>;
+    constexpr int S = GS::S;
+    const int N = kN ? kN : (int)p.n_dim;
+    const int NB = kN ? GS::NB : N;
+
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t local = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
+    if (local >= p.count) return;                          // uniform per warp
+    const uint32_t t_lo = (uint32_t)p.first + local;
+
+    R x[ZMC_MAX_M];
+    decode_point<R>(p, local, static_cast<const R*>(nullptr), x);      // stage_smem is 0 for this kernel
+
+    Fam fam;
+    fam.setup(x, p);
+    PhiloxPoint px;
+    px.init(t_lo, (uint32_t)(p.first >> 32), p.rk);
+
+    uint32_t w[GS::NB * 4];
+    Accum<R> acc;
+    {
+        const int nb0 = (N + 3) >> 2;
+#pragma unroll
+        for (int b = 0; b < (kN ? (kN + 3) / 4 : ZMC_MAX_N / 4); ++b)
+            if (b < nb0) px.block((uint32_t)b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+        acc.K = fam.eval(w);
+    }
+
+    uint32_t n_lo = 0, n_hi = p.n;                          // both multiples of S (validated on the host)
+    double A, B, serr, inv_n;
+    for (;;) {
+        for (uint32_t g = n_lo / S + lane; g < n_hi / S; g += 32u) {
+            const uint32_t j0 = g * (uint32_t)NB;
+            if constexpr (kN != 0) {
+                px.template blocks<GS::NB>(j0, p.rk, w);
+            } else {
+#pragma unroll
+                for (int b = 0; b < GS::NB; ++b)
+                    if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+            }
+#pragma unroll
+            for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
+        }
+        A = acc.A; B = acc.B;                               // lane partials stay put; the tree works on copies
+#pragma unroll
+        for (int m = 16; m >= 1; m >>= 1) {
+            A += __shfl_xor_sync(0xffffffffu, A, m);
+            B += __shfl_xor_sync(0xffffffffu, B, m);
+        }
+        inv_n = 1.0 / (double)n_hi;                         // the same finalisation, operation for operation, as above
+        double m2 = ::fma(-A * inv_n, A, B);
+        m2 = m2 > 0.0 ? m2 : 0.0;
+        serr = p.volume * sqrt(m2 / ((double)(n_hi - 1) * (double)n_hi));
+        if (serr <= p.target || n_hi >= p.n_max) break;    // the same value in every lane: warp-uniform
+        n_lo = n_hi;
+        n_hi = (n_hi > p.n_max - n_hi) ? p.n_max : 2u * n_hi;
+    }
+
+    if (lane == 0) {
+        const double mean = p.volume * ((double)acc.K + A * inv_n);
+        const uint64_t o = p.out_off + local;
+        if (p.out_f32) {
+            static_cast<float*>(out_mean)[o] = (float)mean;
+            static_cast<float*>(out_stderr)[o] = (float)serr;
+        } else {
+            static_cast<double*>(out_mean)[o] = mean;
+            static_cast<double*>(out_stderr)[o] = serr;
+        }
+        p.out_n[o] = n_hi;
+    }
+}
+
 #ifndef __CUDACC_RTC__
 template <class Fam, int SCHED>
 cudaError_t launch_scan(const ScanParams& p, void* out_mean, void* out_stderr, int grid, size_t smem_bytes,
@@ -214,14 +302,24 @@ cudaError_t launch_scan(const ScanParams& p, void* out_mean, void* out_stderr, i
     return cudaGetLastError();
 }
 
-// three table rows (one per schedule) for one family type; the type goes last because it contains commas
+template <class Fam>
+cudaError_t launch_adapt(const ScanParams& p, void* out_mean, void* out_stderr, int grid, size_t smem_bytes,
+                         cudaStream_t stream)
+{
+    zmc_adapt_kernel<Fam><<<grid, kThreads, smem_bytes, stream>>>(p, out_mean, out_stderr);
+    return cudaGetLastError();
+}
+
+// four table rows (the three schedules + the adaptive kernel) for one family type; the type goes last because it contains commas
 #define ZMC_ENTRY(FAMILY_ID, NDIM, PREC, FAST, ...)                                                      \
     {FAMILY_ID, NDIM, PREC, FAST, kSchedThread, &launch_scan<__VA_ARGS__, kSchedThread>,                \
      (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedThread>},                                         \
     {FAMILY_ID, NDIM, PREC, FAST, kSchedWarp, &launch_scan<__VA_ARGS__, kSchedWarp>,                    \
      (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedWarp>},                                           \
     {FAMILY_ID, NDIM, PREC, FAST, kSchedCta, &launch_scan<__VA_ARGS__, kSchedCta>,                      \
-     (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedCta>}
+     (const void*)&zmc_scan_kernel<__VA_ARGS__, kSchedCta>},                                            \
+    {FAMILY_ID, NDIM, PREC, FAST, kSchedAdapt, &launch_adapt<__VA_ARGS__>,                              \
+     (const void*)&zmc_adapt_kernel<__VA_ARGS__>}
 
 // the three arithmetic variants of a family template F<R, ..., FAST>: fp64, fp32+MUFU, fp32 accurate
 #define ZMC_ENTRY_FIXED(FAMILY_ID, NDIM, F)                                  \

@@ -22,10 +22,15 @@ struct ScanParams {
     uint32_t list_off[ZMC_MAX_M]; // offset of list i in `lists`
     double a[ZMC_MAX_N], width[ZMC_MAX_N];   // box; in F32E mode already rounded to float (mirror, reading S5)
     double volume;                // prod_k width_k, k ascending
+    // adaptive scan only (zmc_scan_adaptive, zmc_adapt_kernel): n is the first checkpoint
+    double target;                // stop once stderr <= target ...
+    uint32_t n_max;               // ... or n reaches n_max
+    uint32_t* out_n;              // samples used per point (device), indexed like out_mean
     double consts[ZMC_MAX_CONSTS];
 };
 
-enum { kSchedThread = ZMC_SCHED_THREAD, kSchedWarp = ZMC_SCHED_WARP, kSchedCta = ZMC_SCHED_CTA };
+enum { kSchedThread = ZMC_SCHED_THREAD, kSchedWarp = ZMC_SCHED_WARP, kSchedCta = ZMC_SCHED_CTA,
+       kSchedAdapt = 4 /* internal: the warp-per-point adaptive kernel */ };
 
 constexpr int kThreads = 256;      // CTA size of every schedule
 

@@ -166,10 +166,11 @@ zmc_status zmc_register_integrand(const char* name, const char* body, int N, int
     }
     struct Guard { Nvrtc& rt; nvrtcProgram* p; ~Guard() { rt.destroyProgram(p); } } guard{rt, &prog};
     static const char* kReal[2] = {"double", "float"};
-    std::string expr[2][3];
+    std::string expr[2][4];
     for (int pr = 0; pr < 2; ++pr)
-        for (int sc = 0; sc < 3; ++sc) {
-            expr[pr][sc] = std::string("zmc::zmc_scan_kernel<zmc::FamUser<") + kReal[pr] + ">, " + std::to_string(sc + 1) + ">";
+        for (int sc = 0; sc < 4; ++sc) {
+            expr[pr][sc] = sc < 3 ? std::string("zmc::zmc_scan_kernel<zmc::FamUser<") + kReal[pr] + ">, " + std::to_string(sc + 1) + ">"
+                                  : std::string("zmc::zmc_adapt_kernel<zmc::FamUser<") + kReal[pr] + "> >";
             if (rt.addNameExpression(prog, expr[pr][sc].c_str()) != NVRTC_SUCCESS) {
                 tl_compile_log = "nvrtcAddNameExpression failed";
                 return ZMC_ERR_COMPILE;
@@ -181,6 +182,7 @@ zmc_status zmc_register_integrand(const char* name, const char* body, int N, int
     if (rt.getProgramLogSize(prog, &log_size) == NVRTC_SUCCESS && log_size > 1) {
         tl_compile_log.resize(log_size);
         rt.getProgramLog(prog, &tl_compile_log[0]);
+        while (!tl_compile_log.empty() && tl_compile_log.back() == '\0') tl_compile_log.pop_back();
     }
     if (rc != NVRTC_SUCCESS) return ZMC_ERR_COMPILE;
     size_t cubin_size = 0;
@@ -193,7 +195,7 @@ zmc_status zmc_register_integrand(const char* name, const char* body, int N, int
     cudaError_t e = cudaLibraryLoadData(&u->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
     if (e != cudaSuccess) { tl_compile_log += "\ncudaLibraryLoadData: "; tl_compile_log += cudaGetErrorString(e); return ZMC_ERR_CUDA; }
     for (int pr = 0; pr < 2; ++pr)
-        for (int sc = 0; sc < 3; ++sc) {
+        for (int sc = 0; sc < 4; ++sc) {
             const char* lowered = nullptr;
             if (rt.getLoweredName(prog, expr[pr][sc].c_str(), &lowered) != NVRTC_SUCCESS || !lowered) return ZMC_ERR_COMPILE;
             e = cudaLibraryGetKernel(&u->kern[pr][sc], u->lib, lowered);

@@ -12,7 +12,7 @@ struct UserIntegrand {
     std::string name;
     int N = 0, M = 0, n_consts = 0;
     cudaLibrary_t lib = nullptr;
-    cudaKernel_t kern[2][3] = {};        // [precision][schedule - 1]
+    cudaKernel_t kern[2][4] = {};        // [precision][schedule - 1]; schedule 4 = the adaptive kernel
 };
 
 const UserIntegrand* find_user_integrand(int id);
