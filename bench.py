@@ -169,6 +169,7 @@ def main():
     ap.add_argument("--schedule", type=int, default=0, help="0 auto, 1 thread, 2 warp, 3 cta")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--adaptive", default="", help="n_first,n_max,target_stderr: also time zmc_scan_adaptive (N=1 only)")
     ap.add_argument("--farm-devices", default="", help="e.g. 0,1,2,3: also time zmc_scan_farm over these devices (N=1 only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "zmc" else args.warmup
@@ -278,6 +279,24 @@ def main():
                "d2h_gbs": float(np.mean([i["d2h_bytes"] / max(i["d2h_ms"], 1e-9) * 1e-6 for i in e_infos]))}
         launches += int(sum(i["gpu_launches"] for i in e_infos))
 
+    # ---- NEXT-4: adaptive sample count; throughput counts the samples actually drawn (sum of out_n) -----------------
+    adaptive = None
+    if args.adaptive and world == 1:
+        n_first, n_max, target = args.adaptive.split(",")
+        n_first, n_max, target = int(n_first), int(n_max), float(target)
+        a_n = torch.zeros(count, dtype=torch.int32, device="cuda")
+
+        def step_adaptive():
+            return zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, n_first, n_max, target, w.seed, d_mean, d_err,
+                                        a_n, stream, precision=w.precision, first_index=first, count=count,
+                                        batch_points=w.batch_points, consts=w.consts, timing=True)
+        a_ms, a_infos = timed(step_adaptive, 3, 2)
+        drawn = int(a_n.to(torch.int64).sum().item())
+        adaptive = {"n_first": n_first, "n_max": n_max, "target_stderr": target, "ms_per_step": a_ms / 3,
+                    "samples_drawn": drawn, "value": drawn / (a_ms / 3 * 1e-3), "unit": UNIT,
+                    "mean_n": drawn / count, "frac_at_n_max": float((a_n == n_max).float().mean().item()),
+                    "fixed_n_max_evals": count * n_max}
+
     # ---- NEXT-2: the single-node batch farm over --farm-devices (host outputs, synchronous, host wall clock) -------
     farm = None
     if args.farm_devices and world == 1 and not args.no_e2e:
@@ -312,6 +331,7 @@ def main():
         "clocks": clocks,
         "e2e": e2e,
         "farm": farm,
+        "adaptive": adaptive,
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
                      "frac": achieved / PEAK_GLANE, "traffic": None,
