@@ -22,7 +22,9 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors,
  * the S3 stream values, uniform extremes, param_echo decode, const_one,
  * the n=4 worked example, a pure-Python brute-force enumerator, closed forms
- * of every family (5-sigma coverage, z-score moments, stderr scale).
+ * of every family (5-sigma coverage, z-score moments, stderr scale); the
+ * user-integrand hook (zmc_oracle_set_user) against a closed form
+ * (tests/test_user_integrand_cpu.py).
  * Unpinned: the paper's printed Table-1 delta_r values --
  * "parity unpinned": RNG/seed unspecified by the paper.
  *
