@@ -96,3 +96,30 @@ def test_seed_uses_all_64_bits():
     w.seed = 0x0123456789ABCDEF ^ (1 << 40)
     b, _ = run_gpu(w, schedule=1)
     assert not np.array_equal(a, b)
+
+
+def test_back_to_back_host_output_scans_on_two_streams_and_after_shutdown():
+    """The D2H staging buffers alternate across batches and across calls; several host-output scans in flight at once
+    (different user streams, no synchronisation in between) must not overwrite each other's staged results, and the
+    library must come back after zmc_shutdown()."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    ws = [wl.config(5, scale=[5, 4, 3, 6, 7], n_samples=64 + 8 * i) for i in range(4)]
+    refs = []
+    for w in ws:
+        w.host_out, w.batch_points = False, 0
+        refs.append(run_gpu(w, schedule=1))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = []
+    for i, w in enumerate(ws):                    # four scans enqueued without waiting, 3-5 batches each
+        m = torch.full((w.G,), float("nan"), dtype=torch.float32).pin_memory()
+        e = torch.full((w.G,), float("nan"), dtype=torch.float32).pin_memory()
+        zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, m, e, streams[i & 1], precision=w.precision,
+                       schedule=1, batch_points=600 + 100 * i, consts=w.consts)
+        outs.append((m, e))
+    torch.cuda.synchronize()
+    for (m, e), (rm, re) in zip(outs, refs):
+        assert np.array_equal(m.numpy(), rm) and np.array_equal(e.numpy(), re)
+    zb.zmc_shutdown()
+    m2, e2 = run_gpu(ws[0], schedule=1)
+    assert np.array_equal(m2, refs[0][0]) and np.array_equal(e2, refs[0][1])
