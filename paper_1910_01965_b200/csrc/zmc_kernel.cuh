@@ -126,14 +126,22 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     // pipes instruction by instruction (measured +7 % on cfg2; the one group generated past the end is discarded).
     // fp32 path: FP32 and integer instructions share the dispatch port on sm_100 (profiles/), nothing to overlap.
     if constexpr (kN != 0 && std::is_same<R, double>::value) {
-        uint32_t wn[GS::NB * 4];
+        // two buffers, two groups per iteration: no register copies between "next" and "current"
+        uint32_t wb[GS::NB * 4];
+        const uint32_t step = lanes * (uint32_t)GS::NB;
         uint32_t j0 = lane * (uint32_t)GS::NB;
-        if (lane < n_full) px.template blocks<GS::NB>(j0, p.rk, wn);
-        for (uint32_t g = lane; g < n_full; g += lanes) {
+        if (lane < n_full) px.template blocks<GS::NB>(j0, p.rk, w);
+        uint32_t g = lane;
+        for (; g + lanes < n_full; g += 2u * lanes) {
+            px.template blocks<GS::NB>(j0 + step, p.rk, wb);
 #pragma unroll
-            for (int i = 0; i < GS::NB * 4; ++i) w[i] = wn[i];
-            j0 += lanes * (uint32_t)GS::NB;
-            px.template blocks<GS::NB>(j0, p.rk, wn);
+            for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
+            j0 += 2u * step;
+            px.template blocks<GS::NB>(j0, p.rk, w);
+#pragma unroll
+            for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&wb[s * N], acc.K));
+        }
+        if (g < n_full) {
 #pragma unroll
             for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
         }
