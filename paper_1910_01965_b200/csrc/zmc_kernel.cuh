@@ -16,6 +16,10 @@
 #pragma once
 #include "zmc_families.cuh"
 
+#ifndef ZMC_PIPELINE_F32
+#define ZMC_PIPELINE_F32 0      // measured with the two-buffer loop too: cfg3 -0.2 %, cfg4 -1.4 %, cfg5 -0.5 %
+#endif
+
 
 
 namespace zmc {
@@ -125,7 +129,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     // pipe) sit in the same basic block as the evaluation of the CURRENT one (FP64 pipe), so ptxas alternates the two
     // pipes instruction by instruction (measured +7 % on cfg2; the one group generated past the end is discarded).
     // fp32 path: FP32 and integer instructions share the dispatch port on sm_100 (profiles/), nothing to overlap.
-    if constexpr (kN != 0 && std::is_same<R, double>::value) {
+    if constexpr (kN != 0 && (std::is_same<R, double>::value || ZMC_PIPELINE_F32)) {
         // two buffers, two groups per iteration: no register copies between "next" and "current"
         uint32_t wb[GS::NB * 4];
         const uint32_t step = lanes * (uint32_t)GS::NB;
