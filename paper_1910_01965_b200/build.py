@@ -15,12 +15,14 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-OBJ = os.path.join(HERE, "build")
-LIB = os.path.join(HERE, "libzmc.so")
+# ZMC_VARIANT=<name> builds an experimental copy (extra nvcc flags in ZMC_EXTRA_FLAGS) next to the product library
+VARIANT = os.environ.get("ZMC_VARIANT", "")
+OBJ = os.path.join(HERE, "build" + ("_" + VARIANT if VARIANT else ""))
+LIB = os.path.join(HERE, "libzmc" + ("_" + VARIANT if VARIANT else "") + ".so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 INCLUDE = os.path.normpath(os.path.join(HERE, "..", "include"))
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-I", INCLUDE, "-I", OBJ,
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"] + os.environ.get("ZMC_EXTRA_FLAGS", "").split()
 # headers handed to NVRTC when a user integrand is compiled at run time (zmc_register_integrand): embedded as strings
 RTC_HEADERS = ["zmc_compat.h", "zmc_params.h", "zmc_math.cuh", "zmc_families.cuh", "zmc_kernel.cuh"]
 

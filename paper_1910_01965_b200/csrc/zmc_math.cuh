@@ -12,6 +12,9 @@
 #ifndef ZMC_F64_UNIT_I2F
 #define ZMC_F64_UNIT_I2F 0
 #endif
+#ifndef ZMC_F32_RINT_MAGIC
+#define ZMC_F32_RINT_MAGIC 0
+#endif
 
 namespace zmc {
 
@@ -179,7 +182,12 @@ template <> struct Fn<float, true> {
     static constexpr double kQuarter = 0.25;
     static __device__ __forceinline__ double wrap(double c) { return c - rint(c); }
     static __device__ __forceinline__ float sin_phase(float t) {
+#if ZMC_F32_RINT_MAGIC
+        const float kf = t + 12582912.0f;                                // 1.5 * 2^23: rint(t) in the low mantissa bits
+        const float r = t - (kf - 12582912.0f);                          // 3 FADD, exact for |t| < 2^22, no XU op
+#else
         const float r = t - rintf(t);                                    // FRND (XU pipe) + FADD, exact
+#endif
         return __sinf(r * 6.283185307179586f);                           // FMUL, then FMUL.RZ(1/2pi) + MUFU.SIN
     }
     static __device__ __forceinline__ float sin_phase_minus(float t, float K) { return sin_phase(t) - K; }

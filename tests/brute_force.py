@@ -77,8 +77,34 @@ def _poly(y, x, c):
     return p
 
 
+def _c4(y, x, c):
+    """BASELINE.json configs[3]: g = exp(-sum_k a^2 (y_k - w_k)^2), a = x1,
+    w_k = x2 for k < 2, x3 for 2 <= k < 4, x4 for k >= 4 (k 0-based, reading Q9)."""
+    a = x[0]
+    total = 0.0
+    for k, yk in enumerate(y):
+        if k < 2:
+            wk = x[1]
+        elif k < 4:
+            wk = x[2]
+        else:
+            wk = x[3]
+        total += a * a * (yk - wk) * (yk - wk)
+    return math.exp(-total)
+
+
+def _c5(y, x, c):
+    """BASELINE.json configs[4]: g = exp(-x1 |y|^2) cos(x2 y1 + x3 y2 + x4 y3) (1 + x5 y1 y2 y3) (paper's 1-based y)."""
+    y1, y2, y3 = y
+    x1, x2, x3, x4, x5 = x
+    norm2 = y1 * y1 + y2 * y2 + y3 * y3
+    return math.exp(-x1 * norm2) * math.cos(x2 * y1 + x3 * y2 + x4 * y3) * (1.0 + x5 * y1 * y2 * y3)
+
+
 FAMILIES[6] = _p6
 FAMILIES[3] = _c3
+FAMILIES[4] = _c4
+FAMILIES[5] = _c5
 FAMILIES[103] = _poly
 
 

@@ -80,6 +80,20 @@ def c4_m2(a, w1, w2, w3):
     return c4_mean(np.sqrt(2.0) * a, w1, w2, w3)
 
 
+def _gauss1d_box(a, w, lo, hi):
+    """int_lo^hi exp(-a^2 (y - w)^2) dy."""
+    return np.sqrt(np.pi) / (2 * a) * (special.erf(a * (hi - w)) - special.erf(a * (lo - w)))
+
+
+def c4_mean_box(a, w1, w2, w3, bounds):
+    """c4 over a general box: dimensions 0,1 centre on w1 (= x2), 2,3 on w2 (= x3), 4,5 on w3 (= x4)."""
+    b = np.asarray(bounds, dtype=np.float64).reshape(6, 2)
+    out = 1.0
+    for k, w in enumerate((w1, w1, w2, w2, w3, w3)):
+        out = out * _gauss1d_box(a, w, b[k, 0], b[k, 1])
+    return out
+
+
 # ---- c5: exp(-x1 |y|^2) cos(x2 y1 + x3 y2 + x4 y3) (1 + x5 y1 y2 y3), y in [-1,1]^3 -------
 def J(alpha, c):
     """int_{-1}^{1} exp(-alpha y^2) cos(c y) dy via the complex error function."""
@@ -113,6 +127,25 @@ def c5_m2_scalar(x1, x2, x3, x4, x5):
     t0 = 0.5 * (J_quad(a2, 0.0) ** 3 + J_quad(a2, 2 * x2) * J_quad(a2, 2 * x3) * J_quad(a2, 2 * x4))
     t2 = 0.5 * (_K2(a2, 0.0) ** 3 + _K2(a2, 2 * x2) * _K2(a2, 2 * x3) * _K2(a2, 2 * x4))
     return (t0 + x5 * x5 * t2) / 8.0
+
+
+def _c5_1d(alpha, c, lo, hi, power):
+    """int_lo^hi y^power exp(-alpha y^2 + i c y) dy (complex, quadrature)."""
+    re, _ = integrate.quad(lambda y: y ** power * np.exp(-alpha * y * y) * np.cos(c * y), lo, hi, epsabs=1e-14, epsrel=1e-13)
+    im, _ = integrate.quad(lambda y: y ** power * np.exp(-alpha * y * y) * np.sin(c * y), lo, hi, epsabs=1e-14, epsrel=1e-13)
+    return complex(re, im)
+
+
+def c5_mean_box_scalar(x1, x2, x3, x4, x5, bounds):
+    """c5 over a general box (one parameter point): cos(sum c_k y_k) = Re prod exp(i c_k y_k), so
+    f = Re prod_k A_k + x5 Re prod_k B_k with A_k = int exp(-x1 y^2 + i c_k y), B_k = int y exp(-x1 y^2 + i c_k y).
+    On a box that is not symmetric about 0 the x5 term does NOT vanish: the mean sees x5 and its sign."""
+    b = np.asarray(bounds, dtype=np.float64).reshape(3, 2)
+    A = B = 1.0 + 0.0j
+    for k, c in enumerate((x2, x3, x4)):
+        A *= _c5_1d(x1, c, b[k, 0], b[k, 1], 0)
+        B *= _c5_1d(x1, c, b[k, 0], b[k, 1], 1)
+    return A.real + x5 * B.real
 
 
 # ---- p6: the paper's sin(sum y + sum x) on [0,b]^N (PAPER.md:75, :120) ---------------------

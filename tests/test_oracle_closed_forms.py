@@ -96,6 +96,62 @@ def test_cfg5_reduced_and_x5_independence():
     assert abs(np.mean(ratios) - 1.0) <= 0.1
 
 
+def test_c4_asymmetric_box_pins_which_parameter_centres_which_dimensions():
+    # on [0,1]^6 the integral is symmetric in x2, x3, x4, so the closed form cannot see WHICH
+    # dimensions centre on which parameter.  Box [0,1]^4 x [0,0.5]^2 and different ranges for x3 and x4 break the symmetry
+    # (BASELINE.json configs[3]: w_k = x2 for k<2, x3 for 2<=k<4, x4 for k>=4).
+    bounds = np.array([0.0, 1.0, 0.0, 1.0, 0.0, 1.0, 0.0, 1.0, 0.0, 0.5, 0.0, 0.5])
+    lists = [wl.linspace(1.0, 3.0, 4), wl.linspace(0.1, 0.9, 3), wl.linspace(0.55, 0.95, 4), wl.linspace(0.05, 0.3, 4)]
+    w = wl.Workload("c4_asym", wl.C4_GAUSS_PEAK, bounds, lists, 20000, 44, wl.PREC_F64, np.zeros(0))
+    rc, mean, err = orc.scan_workload(w, n_threads=NT)
+    assert rc == 0
+    a, w1, w2, w3 = cf.grid_params(lists)
+    exact = cf.c4_mean_box(a, w1, w2, w3, bounds)
+    z = (mean - exact) / err
+    assert np.all(np.abs(z) <= 5.0) and abs(z.mean()) <= 4.0 / np.sqrt(len(z)) and abs(z.var() - 1.0) <= 0.45
+    # the test has teeth: with x3 and x4 swapped the closed form is many sigma away at most points
+    swapped = cf.c4_mean_box(a, w1, w3, w2, bounds)
+    assert np.mean(np.abs((mean - swapped) / err) > 5.0) >= 0.9
+
+
+def test_c5_asymmetric_box_mean_sees_x5_and_its_sign():
+    # On [-1,1]^3 the (1 + x5 y0 y1 y2) factor integrates to 1 (oddness), so the cfg 5 closed form is blind to it.
+    # On a box that is not symmetric about 0 it is not: f = Re prod A_k + x5 Re prod B_k (closed_forms.c5_mean_box_scalar).
+    bounds = np.array([0.0, 1.0, -0.5, 1.0, 0.25, 1.5])
+    lists = [np.array([0.3, 1.1]), np.array([0.7]), np.array([1.9]), np.array([0.4, 2.6]), np.array([-3.0, 0.8, 3.5])]
+    w = wl.Workload("c5_asym", wl.C5_DAMPED_COS, bounds, lists, 40000, 55, wl.PREC_F64, np.zeros(0))
+    rc, mean, err = orc.scan_workload(w, n_threads=NT)
+    assert rc == 0
+    xs = cf.grid_params(lists)
+    far = 0
+    for t in range(len(mean)):
+        x = [float(v[t]) for v in xs]
+        exact = cf.c5_mean_box_scalar(*x, bounds)
+        assert abs(mean[t] - exact) <= 5.0 * err[t], (t, x)
+        flipped = cf.c5_mean_box_scalar(x[0], x[1], x[2], x[3], -x[4], bounds)        # wrong sign of the x5 term
+        wrong_par = cf.c5_mean_box_scalar(x[0], x[1], x[2], x[3], x[3], bounds)       # x4 used in place of x5
+        far += int(abs(mean[t] - flipped) > 5.0 * err[t]) + int(abs(mean[t] - wrong_par) > 5.0 * err[t])
+    assert far >= 1.5 * len(mean)        # teeth: both mutations are > 5 sigma away at (at least) three quarters of the points
+
+
+def test_c5_second_moment_per_point_depends_on_x5():
+    # cfg 5's own box: only x5 varies; n stderr^2 / V^2 = Var g must follow E[g^2] = (t0 + x5^2 t2)/8 POINT BY POINT
+    # (a dropped y_k, x4 in place of x5, or a missing factor changes t2's weight; the band is 4 sampling sigma of the variance)
+    w = wl.config(5, scale=[1, 1, 1, 1, 9], n_samples=200_000)
+    w.lists[0] = np.array([0.35]); w.lists[1] = np.array([1.3]); w.lists[2] = np.array([0.6]); w.lists[3] = np.array([2.1])
+    w.lists[4] = wl.linspace(0.1, 8.0, 9)
+    w.precision = wl.PREC_F64
+    rc, mean, err = orc.scan_workload(w, n_threads=NT)
+    assert rc == 0
+    x5s = w.lists[4]
+    exact = float(cf.c5_mean(0.35, 1.3, 0.6, 2.1))
+    got = w.n_samples * err ** 2 / 64.0
+    want = np.array([cf.c5_m2_scalar(0.35, 1.3, 0.6, 2.1, float(x5)) for x5 in x5s]) - (exact / 8.0) ** 2
+    assert np.all(np.abs(got / want - 1.0) <= 0.03), got / want
+    assert want[-1] / want[0] > 2.0      # the x5 term dominates at the top of the list: a version without it fails by a factor
+    assert np.all(np.abs(mean - exact) <= 5.0 * err)
+
+
 @pytest.mark.parametrize("M,N", [(1, 1), (2, 3), (3, 2)])
 def test_paper_eq2_family(M, N):
     # PAPER.md:73-77 Eq. (2) on [0,10]^N; lists {0..L-1}

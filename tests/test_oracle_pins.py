@@ -135,6 +135,12 @@ BF_CASES = [
     (wl.C2_SIN_XY2, [0.0, wl.PI, 0.0, wl.PI], [[0.5, 5.0], [0.5, 2.0, 5.0]], 5, (), False),
     (wl.C3_OSCILLATORY, [0.0, 1.0] * 3, [[0.1, 3.0], [1.0, 2.0], [0.3, 0.7]], 4, (0.25,), False),
     (wl.P6_SIN_SUM, [0.0, 10.0] * 3, [[0.0, 1.0, 2.0], [5.0, 99.0]], 5, (), False),
+    # c4 / c5 with every parameter different (and boxes that differ between the dimension pairs), so that a swapped
+    # parameter, a dropped y_k or a wrong sign changes every sample value
+    (wl.C4_GAUSS_PEAK, [0.0, 1.0, 0.0, 1.0, 0.0, 1.0, 0.0, 1.0, 0.0, 0.5, 0.0, 0.5],
+     [[1.0, 2.5], [0.2], [0.45, 0.7], [0.9, 0.1]], 5, (), False),
+    (wl.C5_DAMPED_COS, [-1.0, 1.0, -1.0, 1.0, -1.0, 1.0], [[0.1, 1.3], [0.7], [2.9, 1.1], [4.0], [3.7, 0.4]], 6, (), False),
+    (wl.C5_DAMPED_COS, [0.0, 1.0, -0.5, 1.0, 0.25, 2.0], [[0.3], [1.7], [0.6], [2.2], [1.9, -2.5]], 7, (), False),
 ]
 
 
