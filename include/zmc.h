@@ -82,6 +82,15 @@ enum { ZMC_OUT_F64 = 0, ZMC_OUT_F32 = 1 };
 enum { ZMC_LOC_DEVICE = 0, ZMC_LOC_HOST = 1 };            /* HOST: pinned memory recommended */
 enum { ZMC_SCHED_AUTO = 0, ZMC_SCHED_THREAD = 1, ZMC_SCHED_WARP = 2, ZMC_SCHED_CTA = 3 };
 enum { ZMC_FAST_MATH_DEFAULT = -1, ZMC_FAST_MATH_OFF = 0, ZMC_FAST_MATH_ON = 1 };
+/* zmc_options.flags */
+enum {
+    ZMC_OPT_EXPLICIT_COUNT = 1,   /* take `count` literally: count == 0 is an EMPTY range (nothing enqueued, nothing written)
+                                     instead of "up to the end of the grid" -- for callers whose shard may be empty */
+    ZMC_OPT_FRESH_LISTS = 2       /* upload the value lists even if an identical copy is cached on the device (timing runs
+                                     that must contain the HToD copy) */
+};
+/* zmc_register_integrand_ex flags */
+enum { ZMC_USER_FAST_MATH = 1 };  /* compile the user body with NVRTC --use_fast_math (fp32 only: sinf -> MUFU etc.) */
 
 /* One parameter's value list.  Host memory. */
 typedef struct zmc_param_list {
@@ -99,15 +108,15 @@ typedef struct zmc_options {
     int32_t fast_math;       /* ZMC_FAST_MATH_*: F32E only -- MUFU sin/cos/ex2 (default ON); ignored for F64 */
     uint64_t batch_points;   /* grid points per batch; 0 = one batch */
     uint64_t first_index;    /* scan only flat indices [first_index, first_index+count) ... */
-    uint64_t count;          /* ... 0 = up to the end of the grid */
+    uint64_t count;          /* ... 0 = up to the end of the grid (unless flags has ZMC_OPT_EXPLICIT_COUNT: then 0 = empty) */
     const double* consts;    /* family constants (host), n_consts of them */
     int32_t n_consts;
-    int32_t reserved;
+    int32_t flags;           /* ZMC_OPT_* bits, 0 = none */
 } zmc_options;
 
 /* Where the time went (the paper's HToD / DToH / GPU evaluation split). */
 typedef struct zmc_timing {
-    double h2d_ms;           /* staging of bounds/lists (device time) */
+    double h2d_ms;           /* staging of the value lists (device time; ~0 when the lists were already cached on the device) */
     double kernel_ms;        /* sum of the batch kernels' device time */
     double d2h_ms;           /* sum of the result copies' device time (host output only) */
     double exposed_d2h_ms;   /* max(0, wall - h2d - kernel): copy time NOT hidden behind compute */
@@ -115,9 +124,10 @@ typedef struct zmc_timing {
     int64_t n_batches;
     int64_t gpu_launches;    /* kernels of this library launched by the call */
     uint64_t d2h_bytes;
-    uint64_t h2d_bytes;
+    uint64_t h2d_bytes;      /* bytes this call copied host -> device (0 on a list-cache hit) */
     int32_t schedule;        /* the schedule actually used */
-    int32_t reserved;
+    int32_t host_out_pinned; /* HOST outputs: 1 = page-locked (copies overlap compute), 0 = pageable (cudaMemcpyAsync then runs
+                                synchronously on the host: no overlap, exposed_d2h_ms is the whole copy); -1 = device outputs */
 } zmc_timing;
 
 /* What zmc_scan_farm did (the paper's allocation / evaluation view of Table 2). Host wall clock. */
@@ -130,6 +140,21 @@ typedef struct zmc_farm_timing {
     int64_t batches_done[ZMC_MAX_FARM_DEVICES];      /* batches each device slot ended up taking (dynamic assignment) */
     double busy_ms[ZMC_MAX_FARM_DEVICES];            /* first pull to last completion, per device slot */
 } zmc_farm_timing;
+
+/* zmc_measure_pipes: one measured row.  All three numbers are SM-sub-partition cycles per group of instructions per warp. */
+#define ZMC_PIPE_MAX_ROWS 48
+typedef struct zmc_pipe_row {
+    char name[72];           /* e.g. "LOP3", "1xIMAD.WIDE+LOP3 + 2xDFMA, same warp", "cfg2 block: both, same warp (ptxas order)" */
+    double cycles;           /* measured */
+    double parallel;         /* max of the parts' own costs: what independent pipes would give */
+    double serial;           /* sum of the parts' own costs: what one shared pipe would give */
+} zmc_pipe_row;
+typedef struct zmc_pipe_report {
+    double sm_mhz;           /* SM clock while measuring (clock64 against globaltimer) */
+    int32_t sm_count;
+    int32_t n_rows;
+    zmc_pipe_row rows[ZMC_PIPE_MAX_ROWS];
+} zmc_pipe_report;
 
 typedef struct zmc_integrand_info {
     int32_t id;
@@ -169,8 +194,10 @@ ZMC_API const char* zmc_version(void);
 /* Validate arguments exactly as zmc_scan_ex does, enqueue nothing; writes G (whole grid) if non-NULL. */
 ZMC_API zmc_status zmc_validate(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                         uint64_t n_samples, const zmc_options* opt, uint64_t* grid_points);
-/* The schedule AUTO would pick for `count` points of `n_samples` samples in N dimensions. */
+/* The schedule AUTO would pick for `count` points of `n_samples` samples in N dimensions (fp64 path; _ex: either
+ * precision -- the fp32-evaluate kernels keep more threads resident, so their thresholds are higher). */
 ZMC_API int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N);
+ZMC_API int zmc_pick_schedule_ex(uint64_t count, uint64_t n_samples, int N, int precision);
 /* Batch b of a range cut into batches of batch_points: writes its (first, count). Returns the number of batches. */
 ZMC_API int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t batch_points, int64_t b,
                         uint64_t* batch_first, uint64_t* batch_count);
@@ -182,9 +209,10 @@ ZMC_API int64_t zmc_batch_range(uint64_t first_index, uint64_t count, uint64_t b
  * a checkpoint uses exactly the first n samples: the outputs equal zmc_scan_ex(n_samples = out_n[point],
  * schedule = ZMC_SCHED_WARP) bit for bit.
  *   n_first   first checkpoint, a multiple of 256 (>= 256)      n_max  last checkpoint, a multiple of 8, >= n_first
- *   out_n     samples used per point (uint32, DEVICE memory, indexed like out_mean)
- * Outputs must be DEVICE memory (opt->out_location); opt->schedule is ignored (one warp per point); batching, sub-ranges,
- * precision, out_dtype and timing behave as in zmc_scan_ex.
+ *   out_n     samples used per point (uint32, indexed like out_mean, in the SAME memory as out_mean: device, or host
+ *             with opt->out_location = ZMC_LOC_HOST -- it is then streamed batch by batch with the results)
+ * opt->schedule is ignored (one warp per point); batching, sub-ranges, precision, out_dtype, out_location and timing behave
+ * as in zmc_scan_ex.
  */
 ZMC_API zmc_status zmc_scan_adaptive(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                              uint64_t n_first, uint64_t n_max, double target_stderr, uint64_t seed, void* out_mean,
@@ -203,6 +231,13 @@ ZMC_API zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, 
                          uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, const int* devices,
                          int n_devices, const zmc_options* opt, zmc_farm_timing* timing);
 
+/* zmc_scan_farm with a per-point adaptive sample count (zmc_scan_adaptive's n_first / n_max / target_stderr); out_n is a
+ * host array like out_mean.  Bit-identical to zmc_scan_adaptive on one device. */
+ZMC_API zmc_status zmc_scan_farm_adaptive(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                                  uint64_t n_first, uint64_t n_max, double target_stderr, uint64_t seed, void* out_mean,
+                                  void* out_stderr, uint32_t* out_n, const int* devices, int n_devices,
+                                  const zmc_options* opt, zmc_farm_timing* timing);
+
 /*
  * zmc_register_integrand -- a user-defined integrand ("users have a full flexibility to define their own
  * integrands", :49, :162; the paper JIT-compiles a Python function, here it is CUDA C++ compiled with NVRTC for
@@ -212,12 +247,33 @@ ZMC_API zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, 
  *          c: the n_consts constants of zmc_options.consts; R is double (ZMC_PREC_F64) or float (ZMC_PREC_F32E).
  *          Example: "return exp(-x[0] * y[0] * y[0]) * cos(x[1] * y[1] + c[0]);"
  *   N, M, n_consts   the shape the integrand accepts (anything else is ZMC_ERR_SHAPE_MISMATCH at scan time)
- *   integrand_id     out: an id >= 1000 to pass to zmc_scan / zmc_scan_ex (valid until zmc_shutdown)
- * Host strings are copied.  ZMC_ERR_COMPILE: libnvrtc.so.12 not found or compilation failed (log below);
- * ZMC_ERR_CUDA: compiled, but the code could not be loaded (no usable device).  fast_math is ignored for user integrands.
+ *   integrand_id     out: an id >= 1000 to pass to zmc_scan / zmc_scan_ex (valid until zmc_unregister_integrand / zmc_shutdown)
+ * The body may call the transcendentals the built-in families use (branch-free, no table loads, no slow path), overloaded
+ * for R = double and R = float:  zmc_sin(v) zmc_cos(v) [radians], zmc_sinpi(v) zmc_cospi(v) [argument in units of pi],
+ * zmc_exp(v), zmc_exp2(v).  double: sin/cos to |error| <= 3e-16 (1 + |v|) (own polynomial after an exact reduction),
+ * exp/exp2 = libdevice.  float: sinf/cosf/expf accuracy by default; with ZMC_USER_FAST_MATH (zmc_register_integrand_ex)
+ * the MUFU forms after an exact range reduction (absolute error ~1e-6) and NVRTC --use_fast_math for the rest of the body.
+ * Plain sin()/cos()/exp() work too (libdevice), at about half the speed in fp64.
+ * Compiled integrands are CACHED by the hash of (body, N, M, n_consts, flags): registering the same integrand again costs
+ * microseconds and returns the same id.  Host strings are copied.  ZMC_ERR_COMPILE: libnvrtc.so.12 not found or compilation
+ * failed (log below); ZMC_ERR_CUDA: compiled, but the code could not be loaded (no usable device).  zmc_options.fast_math is
+ * ignored for user integrands (use ZMC_USER_FAST_MATH at registration).
  */
 ZMC_API zmc_status zmc_register_integrand(const char* name, const char* body, int N, int M, int n_consts, int* integrand_id);
+ZMC_API zmc_status zmc_register_integrand_ex(const char* name, const char* body, int N, int M, int n_consts, int flags,
+                                     int* integrand_id);
+/* Forget a user integrand and unload its code.  No scan using it may be in flight.  ZMC_ERR_UNKNOWN_INTEGRAND if not registered. */
+ZMC_API zmc_status zmc_unregister_integrand(int integrand_id);
 ZMC_API const char* zmc_last_compile_log(void);   /* NVRTC log of the last zmc_register_integrand on this thread */
+/*
+ * zmc_measure_pipes -- the roofline denominators of the hot loop, measured on the current device (the
+ * loop is bound by ALU dispatch, "re-measure by micro-benchmark, these are the denominators").  Runs ~35 short synthetic
+ * kernels (about 0.1 s) on `stream` and synchronises: the dispatch cost of every instruction class the loop uses, which
+ * pairs of classes overlap (in one warp, and across warps), and cfg 2's instruction mix per Philox block.
+ * section 6 explains how the ALU roofline is built from these rows; bench.py embeds them in its JSON line.
+ */
+ZMC_API zmc_status zmc_measure_pipes(zmc_pipe_report* report, void* stream);
+
 /* Free the cached per-device scratch (staging buffers, streams, events) and unload user integrands. */
 ZMC_API void zmc_shutdown(void);
 #endif /* !__CUDACC_RTC__ */

@@ -59,7 +59,12 @@ def set_user_integrand(c_body: str, N: int, M: int, n_consts: int = 0):
     import hashlib
     import subprocess
     import tempfile
-    src = ("#include <math.h>\n#define R double\n"
+    # the helper names include/zmc.h offers to user bodies (zmc_register_integrand), by their plain definitions
+    helpers = ("static double zmc_sin(double v) { return sin(v); }\nstatic double zmc_cos(double v) { return cos(v); }\n"
+               "static double zmc_sinpi(double v) { return sin(3.141592653589793 * v); }\n"
+               "static double zmc_cospi(double v) { return cos(3.141592653589793 * v); }\n"
+               "static double zmc_exp(double v) { return exp(v); }\nstatic double zmc_exp2(double v) { return exp2(v); }\n")
+    src = ("#include <math.h>\n#define R double\n" + helpers +
            "double zmc_user_g(const double* y, const double* x, const double* c) {\n" + c_body + "\n}\n")
     d = os.path.join(tempfile.gettempdir(), "zmc_oracle_user")
     os.makedirs(d, exist_ok=True)
@@ -67,7 +72,8 @@ def set_user_integrand(c_body: str, N: int, M: int, n_consts: int = 0):
     if not os.path.exists(base + ".so"):
         with open(base + ".c", "w") as f:
             f.write(src)
-        subprocess.run(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-shared", "-fPIC", base + ".c", "-o", base + ".so", "-lm"],
+        subprocess.run(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-Wno-unused-function", "-shared", "-fPIC", base + ".c",
+                        "-o", base + ".so", "-lm"],
                        check=True)
     so = ctypes.CDLL(base + ".so")
     fn = ctypes.cast(so.zmc_user_g, USER_FN)

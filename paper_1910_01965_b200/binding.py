@@ -25,11 +25,15 @@ ZMC_OUT_F64, ZMC_OUT_F32 = 0, 1
 ZMC_LOC_DEVICE, ZMC_LOC_HOST = 0, 1
 ZMC_SCHED_AUTO, ZMC_SCHED_THREAD, ZMC_SCHED_WARP, ZMC_SCHED_CTA = 0, 1, 2, 3
 ZMC_FAST_MATH_DEFAULT, ZMC_FAST_MATH_OFF, ZMC_FAST_MATH_ON = -1, 0, 1
+ZMC_OPT_EXPLICIT_COUNT, ZMC_OPT_FRESH_LISTS = 1, 2
+ZMC_USER_FAST_MATH = 1
 
 EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info_at",
            "zmc_integrand_info_by_id", "zmc_status_string", "zmc_last_cuda_error", "zmc_version",
            "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown",
-           "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm", "zmc_scan_adaptive"]
+           "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm", "zmc_scan_adaptive",
+           "zmc_pick_schedule_ex", "zmc_register_integrand_ex", "zmc_unregister_integrand", "zmc_scan_farm_adaptive",
+           "zmc_measure_pipes"]
 
 
 class zmc_param_list(ctypes.Structure):
@@ -41,17 +45,17 @@ class zmc_options(ctypes.Structure):
                 ("out_location", ctypes.c_int32), ("schedule", ctypes.c_int32), ("fast_math", ctypes.c_int32),
                 ("batch_points", ctypes.c_uint64), ("first_index", ctypes.c_uint64), ("count", ctypes.c_uint64),
                 ("consts", ctypes.POINTER(ctypes.c_double)), ("n_consts", ctypes.c_int32),
-                ("reserved", ctypes.c_int32)]
+                ("flags", ctypes.c_int32)]
 
 
 class zmc_timing(ctypes.Structure):
     _fields_ = [("h2d_ms", ctypes.c_double), ("kernel_ms", ctypes.c_double), ("d2h_ms", ctypes.c_double),
                 ("exposed_d2h_ms", ctypes.c_double), ("wall_ms", ctypes.c_double), ("n_batches", ctypes.c_int64),
                 ("gpu_launches", ctypes.c_int64), ("d2h_bytes", ctypes.c_uint64), ("h2d_bytes", ctypes.c_uint64),
-                ("schedule", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("schedule", ctypes.c_int32), ("host_out_pinned", ctypes.c_int32)]
 
     def as_dict(self):
-        return {f: getattr(self, f) for f, _ in self._fields_ if f != "reserved"}
+        return {f: getattr(self, f) for f, _ in self._fields_}
 
 
 ZMC_MAX_FARM_DEVICES = 16
@@ -61,6 +65,19 @@ class zmc_farm_timing(ctypes.Structure):
     _fields_ = [("wall_ms", ctypes.c_double), ("n_batches", ctypes.c_int64), ("batch_points", ctypes.c_uint64),
                 ("n_devices", ctypes.c_int32), ("reserved", ctypes.c_int32),
                 ("batches_done", ctypes.c_int64 * ZMC_MAX_FARM_DEVICES), ("busy_ms", ctypes.c_double * ZMC_MAX_FARM_DEVICES)]
+
+
+ZMC_PIPE_MAX_ROWS = 48
+
+
+class zmc_pipe_row(ctypes.Structure):
+    _fields_ = [("name", ctypes.c_char * 72), ("cycles", ctypes.c_double), ("parallel", ctypes.c_double),
+                ("serial", ctypes.c_double)]
+
+
+class zmc_pipe_report(ctypes.Structure):
+    _fields_ = [("sm_mhz", ctypes.c_double), ("sm_count", ctypes.c_int32), ("n_rows", ctypes.c_int32),
+                ("rows", zmc_pipe_row * ZMC_PIPE_MAX_ROWS)]
 
 
 class zmc_integrand_info(ctypes.Structure):
@@ -79,17 +96,22 @@ _lib = None
 
 
 def load():
-    """Load libzmc.so (building it with nvcc if it is missing).  Raises if that is impossible."""
+    """Load libzmc.so.  The mtime-checked build runs first, so a library that is older than its sources is never loaded
+    silently (the .so travels to GPU boxes although git ignores it).  Raises if there is no usable library."""
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
+    default_path = os.path.join(_HERE, "libzmc.so")
+    if LIB_PATH == default_path:
         try:
             from . import build as _build
             _build.build()
         except Exception as exc:  # noqa: BLE001
-            raise RuntimeError(f"libzmc.so is missing and could not be built ({exc}); "
-                               "run `python -m paper_1910_01965_b200.build` -- there is no CPU fallback") from exc
+            if not os.path.exists(LIB_PATH):
+                raise RuntimeError(f"libzmc.so is missing and could not be built ({exc}); "
+                                   "run `python -m paper_1910_01965_b200.build` -- there is no CPU fallback") from exc
+            import warnings
+            warnings.warn(f"libzmc.so could not be rebuilt ({exc}); loading the existing one, which may be stale")
     lib = ctypes.CDLL(LIB_PATH)
     P = ctypes.POINTER
     scan_args = [ctypes.c_int, ctypes.c_int, P(ctypes.c_double), ctypes.c_int, P(zmc_param_list),
@@ -110,6 +132,8 @@ def load():
     lib.zmc_validate.restype = ctypes.c_int
     lib.zmc_pick_schedule.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int]
     lib.zmc_pick_schedule.restype = ctypes.c_int
+    lib.zmc_pick_schedule_ex.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, ctypes.c_int]
+    lib.zmc_pick_schedule_ex.restype = ctypes.c_int
     lib.zmc_batch_range.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int64,
                                     P(ctypes.c_uint64), P(ctypes.c_uint64)]
     lib.zmc_batch_range.restype = ctypes.c_int64
@@ -118,12 +142,23 @@ def load():
                                            P(ctypes.c_int)]
     lib.zmc_register_integrand.restype = ctypes.c_int
     lib.zmc_last_compile_log.restype = ctypes.c_char_p
+    lib.zmc_register_integrand_ex.argtypes = [ctypes.c_char_p, ctypes.c_char_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                              ctypes.c_int, P(ctypes.c_int)]
+    lib.zmc_register_integrand_ex.restype = ctypes.c_int
+    lib.zmc_unregister_integrand.argtypes = [ctypes.c_int]
+    lib.zmc_unregister_integrand.restype = ctypes.c_int
+    lib.zmc_measure_pipes.argtypes = [P(zmc_pipe_report), ctypes.c_void_p]
+    lib.zmc_measure_pipes.restype = ctypes.c_int
     lib.zmc_scan_farm.argtypes = scan_args[:9] + [P(ctypes.c_int), ctypes.c_int, P(zmc_options), P(zmc_farm_timing)]
     lib.zmc_scan_farm.restype = ctypes.c_int
     lib.zmc_scan_adaptive.argtypes = scan_args[:5] + [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_double, ctypes.c_uint64,
                                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                                       P(zmc_options), P(zmc_timing)]
     lib.zmc_scan_adaptive.restype = ctypes.c_int
+    lib.zmc_scan_farm_adaptive.argtypes = scan_args[:5] + [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_double, ctypes.c_uint64,
+                                                           ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, P(ctypes.c_int),
+                                                           ctypes.c_int, P(zmc_options), P(zmc_farm_timing)]
+    lib.zmc_scan_farm_adaptive.restype = ctypes.c_int
     _lib = lib
     return lib
 
@@ -165,7 +200,7 @@ class _Marshalled:
 
 
 def _make_options(m: _Marshalled, precision, out_dtype, out_location, schedule, fast_math, batch_points,
-                  first_index, count) -> zmc_options:
+                  first_index, count, flags: int = 0) -> zmc_options:
     o = zmc_options()
     o.struct_size = ctypes.sizeof(zmc_options)
     o.precision, o.out_dtype, o.out_location = precision, out_dtype, out_location
@@ -173,7 +208,22 @@ def _make_options(m: _Marshalled, precision, out_dtype, out_location, schedule, 
     o.batch_points, o.first_index, o.count = batch_points, first_index, count
     o.consts = m.consts_ptr()
     o.n_consts = len(m.consts)
+    o.flags = flags
     return o
+
+
+_warned_pageable = False
+
+
+def _warn_pageable():
+    """HOST outputs in pageable memory: cudaMemcpyAsync then runs synchronously on the host, so the copy of batch b
+    does not overlap the kernel of batch b+1 (zmc_timing.host_out_pinned reports 0).  Said once."""
+    global _warned_pageable
+    if not _warned_pageable:
+        import warnings
+        warnings.warn("zmc: host output buffers are pageable; result copies will not overlap compute -- pass pinned "
+                      "memory (torch.empty(..., pin_memory=True)) for streaming scans", stacklevel=3)
+        _warned_pageable = True
 
 
 def _tensor_ptr(t):
@@ -181,10 +231,13 @@ def _tensor_ptr(t):
     if isinstance(t, np.ndarray):
         dt = {np.dtype(np.float64): ZMC_OUT_F64, np.dtype(np.float32): ZMC_OUT_F32}[t.dtype]
         assert t.flags["C_CONTIGUOUS"]
+        _warn_pageable()
         return t.ctypes.data, dt, ZMC_LOC_HOST
     import torch
     assert t.is_contiguous()
     dt = {torch.float64: ZMC_OUT_F64, torch.float32: ZMC_OUT_F32}[t.dtype]
+    if not t.is_cuda and not t.is_pinned():
+        _warn_pageable()
     return t.data_ptr(), dt, (ZMC_LOC_DEVICE if t.is_cuda else ZMC_LOC_HOST)
 
 
@@ -211,7 +264,7 @@ def zmc_scan(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_me
 def zmc_scan_ex(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, stream=None, *,
                 precision: int = ZMC_PREC_F64, schedule: int = ZMC_SCHED_AUTO,
                 fast_math: int = ZMC_FAST_MATH_DEFAULT, batch_points: int = 0, first_index: int = 0,
-                count: int = 0, consts=None, timing: bool = False) -> Optional[dict]:
+                count: int = 0, consts=None, timing: bool = False, flags: int = 0) -> Optional[dict]:
     """include/zmc.h zmc_scan_ex.  Output dtype/location are taken from the output tensors
     (torch CUDA tensor = DEVICE; torch CPU tensor or numpy array = HOST).  Returns the timing
     dict when timing=True (the call then synchronises), else None."""
@@ -220,7 +273,7 @@ def zmc_scan_ex(integrand_id: int, bounds, lists, n_samples: int, seed: int, out
     pe, de, le = _tensor_ptr(out_stderr)
     if (dm, lm) != (de, le):
         raise ZmcError(ZMC_ERR_INVALID_ARG, "out_mean and out_stderr must share dtype and location")
-    o = _make_options(m, precision, dm, lm, schedule, fast_math, batch_points, first_index, count)
+    o = _make_options(m, precision, dm, lm, schedule, fast_math, batch_points, first_index, count, flags)
     tm = zmc_timing() if timing else None
     _check(load().zmc_scan_ex(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_samples, seed,
                               ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(_stream_handle(stream)),
@@ -241,8 +294,38 @@ def zmc_validate(integrand_id: int, bounds, lists, n_samples: int, *, precision:
     return int(st), int(g.value)
 
 
-def zmc_pick_schedule(count: int, n_samples: int, N: int) -> int:
-    return int(load().zmc_pick_schedule(count, n_samples, N))
+def zmc_pick_schedule(count: int, n_samples: int, N: int, precision: Optional[int] = None) -> int:
+    if precision is None:
+        return int(load().zmc_pick_schedule(count, n_samples, N))
+    return int(load().zmc_pick_schedule_ex(count, n_samples, N, precision))
+
+
+class ScanPlan:
+    """The arguments of one zmc_scan_ex call, marshalled once.  Calling the plan is a single ctypes call, so a loop over a
+    small grid (cfg 1: the kernel runs 25 us) does not pay the numpy conversions again.  Marshalling only: the plan holds
+    pointers and sizes, nothing is computed here."""
+
+    def __init__(self, integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, *,
+                 precision: int = ZMC_PREC_F64, schedule: int = ZMC_SCHED_AUTO, fast_math: int = ZMC_FAST_MATH_DEFAULT,
+                 batch_points: int = 0, first_index: int = 0, count: int = 0, consts=None, flags: int = 0):
+        self._m = _Marshalled(bounds, lists, consts)
+        pm, dm, lm = _tensor_ptr(out_mean)
+        pe, de, le = _tensor_ptr(out_stderr)
+        if (dm, lm) != (de, le):
+            raise ZmcError(ZMC_ERR_INVALID_ARG, "out_mean and out_stderr must share dtype and location")
+        self._keep = (out_mean, out_stderr)
+        self._o = _make_options(self._m, precision, dm, lm, schedule, fast_math, batch_points, first_index, count, flags)
+        self._tm = zmc_timing()
+        self._fn = load().zmc_scan_ex
+        self._args = (integrand_id, self._m.N, self._m.bounds_ptr(), self._m.M, self._m.c_lists, n_samples, seed,
+                      ctypes.c_void_p(pm), ctypes.c_void_p(pe))
+
+    def __call__(self, stream=None, timing: bool = False) -> Optional[dict]:
+        st = self._fn(*self._args, ctypes.c_void_p(_stream_handle(stream)), ctypes.byref(self._o),
+                      ctypes.byref(self._tm) if timing else None)
+        if st != ZMC_OK:
+            _check(st)
+        return self._tm.as_dict() if timing else None
 
 
 def zmc_batch_range(first_index: int, count: int, batch_points: int, b: int):
@@ -272,8 +355,8 @@ def zmc_scan_adaptive(integrand_id: int, bounds, lists, n_first: int, n_max: int
     m = _Marshalled(bounds, lists, consts)
     pm, dm, lm = _tensor_ptr(out_mean)
     pe, de, le = _tensor_ptr(out_stderr)
-    if (dm, lm) != (de, le) or not out_n.is_cuda or out_n.element_size() != 4:
-        raise ZmcError(ZMC_ERR_INVALID_ARG, "outputs must share dtype/location; out_n must be a 4-byte CUDA tensor")
+    if (dm, lm) != (de, le) or out_n.element_size() != 4 or out_n.is_cuda != (lm == ZMC_LOC_DEVICE):
+        raise ZmcError(ZMC_ERR_INVALID_ARG, "outputs must share dtype/location; out_n must be a 4-byte tensor in the same memory")
     o = _make_options(m, precision, dm, lm, ZMC_SCHED_AUTO, fast_math, batch_points, first_index, count)
     tm = zmc_timing() if timing else None
     _check(load().zmc_scan_adaptive(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_first, n_max, target_stderr, seed,
@@ -303,12 +386,48 @@ def zmc_scan_farm(integrand_id: int, bounds, lists, n_samples: int, seed: int, o
             "batches_done": list(tm.batches_done[:n]), "busy_ms": list(tm.busy_ms[:n])}
 
 
-def zmc_register_integrand(name: str, body: str, N: int, M: int, n_consts: int = 0) -> int:
+def zmc_scan_farm_adaptive(integrand_id: int, bounds, lists, n_first: int, n_max: int, target_stderr: float, seed: int,
+                           out_mean, out_stderr, out_n, devices, *, precision: int = ZMC_PREC_F64,
+                           fast_math: int = ZMC_FAST_MATH_DEFAULT, batch_points: int = 0, first_index: int = 0,
+                           count: int = 0, consts=None) -> dict:
+    """zmc_scan_adaptive farmed over several GPUs (host outputs incl. out_n, synchronous)."""
+    lib = load()
+    m = _Marshalled(bounds, lists, consts)
+    pm, dt_m, loc_m = _tensor_ptr(out_mean)
+    pe, dt_e, loc_e = _tensor_ptr(out_stderr)
+    if dt_m != dt_e or loc_m != ZMC_LOC_HOST or loc_e != ZMC_LOC_HOST or out_n.is_cuda or out_n.element_size() != 4:
+        raise ValueError("zmc_scan_farm_adaptive needs host arrays (mean/stderr of one dtype, out_n 4-byte)")
+    o = _make_options(m, precision, dt_m, ZMC_LOC_HOST, ZMC_SCHED_AUTO, fast_math, batch_points, first_index, count)
+    devs = (ctypes.c_int * len(devices))(*devices)
+    tm = zmc_farm_timing()
+    _check(lib.zmc_scan_farm_adaptive(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_first, n_max, target_stderr, seed,
+                                      ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(out_n.data_ptr()), devs,
+                                      len(devices), ctypes.byref(o), ctypes.byref(tm)))
+    n = tm.n_devices
+    return {"wall_ms": tm.wall_ms, "n_batches": tm.n_batches, "batch_points": tm.batch_points, "n_devices": n,
+            "batches_done": list(tm.batches_done[:n]), "busy_ms": list(tm.busy_ms[:n])}
+
+
+def zmc_measure_pipes(stream=None) -> dict:
+    """include/zmc.h zmc_measure_pipes: the measured dispatch costs behind the ALU roofline."""
+    rep = zmc_pipe_report()
+    _check(load().zmc_measure_pipes(ctypes.byref(rep), ctypes.c_void_p(_stream_handle(stream))))
+    return {"sm_mhz": rep.sm_mhz, "sm_count": rep.sm_count,
+            "rows": [{"name": rep.rows[i].name.decode(), "cycles": rep.rows[i].cycles, "parallel": rep.rows[i].parallel,
+                      "serial": rep.rows[i].serial} for i in range(rep.n_rows)]}
+
+
+def zmc_unregister_integrand(integrand_id: int):
+    _check(load().zmc_unregister_integrand(integrand_id))
+
+
+def zmc_register_integrand(name: str, body: str, N: int, M: int, n_consts: int = 0, flags: int = 0) -> int:
     """Compile a user integrand (body of `template <typename R> __device__ R g(const R* y, const R* x, const R* c)`)
-    with NVRTC; returns its integrand id.  Raises ZmcError (status ZMC_ERR_COMPILE carries the NVRTC log)."""
+    with NVRTC; returns its integrand id (the cached one if this integrand was registered before).  Raises ZmcError
+    (status ZMC_ERR_COMPILE carries the NVRTC log)."""
     lib = load()
     out = ctypes.c_int(0)
-    st = lib.zmc_register_integrand(name.encode(), body.encode(), N, M, n_consts, ctypes.byref(out))
+    st = lib.zmc_register_integrand_ex(name.encode(), body.encode(), N, M, n_consts, flags, ctypes.byref(out))
     if st != ZMC_OK:
         log = (lib.zmc_last_compile_log() or b"").decode(errors="replace")
         raise ZmcError(st, lib.zmc_status_string(st).decode() + (": " + log[-2000:] if log else ""))
@@ -334,7 +453,7 @@ def zmc_shutdown():
 def scan_workload(w, *, schedule: int = ZMC_SCHED_AUTO, fast_math: int = ZMC_FAST_MATH_DEFAULT,
                   first_index: int = 0, count: int = 0, batch_points: Optional[int] = None,
                   host_out: Optional[bool] = None, out_mean=None, out_stderr=None, timing: bool = False,
-                  stream=None):
+                  stream=None, flags: int = 0):
     """Convenience for tests/bench: run a workloads.Workload; allocates the outputs (torch) unless given.
     Returns (out_mean, out_stderr, timing_dict_or_None); outputs are valid after the stream is synchronised."""
     import torch
@@ -351,5 +470,5 @@ def scan_workload(w, *, schedule: int = ZMC_SCHED_AUTO, fast_math: int = ZMC_FAS
     tm = zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, out_mean, out_stderr, stream,
                      precision=w.precision, schedule=schedule, fast_math=fast_math,
                      batch_points=w.batch_points if batch_points is None else batch_points,
-                     first_index=first_index, count=count, consts=w.consts, timing=timing)
+                     first_index=first_index, count=count, consts=w.consts, timing=timing, flags=flags)
     return out_mean, out_stderr, tm

@@ -11,13 +11,15 @@
 #include <thread>
 #include <vector>
 
+#include "zmc_internal.h"
 #include "zmc_params.h"
 
-extern "C" {
+namespace {
 
-zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
-                         uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, const int* devices,
-                         int n_devices, const zmc_options* opt, zmc_farm_timing* timing) {
+// n_samples is the fixed sample count, or (ad != nullptr) the first checkpoint of the adaptive scan
+zmc_status farm_impl(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                     uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, const zmc::AdaptArgs* ad,
+                     const int* devices, int n_devices, const zmc_options* opt, zmc_farm_timing* timing) {
     if (!devices || n_devices < 1 || n_devices > ZMC_MAX_FARM_DEVICES || !out_mean || !out_stderr) return ZMC_ERR_INVALID_ARG;
     zmc_options o;
     std::memset(&o, 0, sizeof(o));
@@ -37,11 +39,11 @@ zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, c
         if (devices[d] < 0 || devices[d] >= n_visible) return ZMC_ERR_INVALID_ARG;
 
     const uint64_t first = o.first_index;
-    const uint64_t count = o.count ? o.count : G - first;
+    const uint64_t count = (o.count || (o.flags & ZMC_OPT_EXPLICIT_COUNT)) ? o.count : G - first;
     if (timing) std::memset(timing, 0, sizeof(*timing));
     if (count == 0) return ZMC_OK;
     // AUTO is resolved once, from the whole range, so that every batch sums in the same order as a one-device scan
-    if (o.schedule == ZMC_SCHED_AUTO) o.schedule = zmc_pick_schedule(count, n_samples, N);
+    if (o.schedule == ZMC_SCHED_AUTO) o.schedule = zmc_pick_schedule_ex(count, n_samples, N, o.precision);
     // default batch: ~8 batches per device so a slow device does not hold the tail (18 s vs 89 s per batch)
     uint64_t bp = o.batch_points ? o.batch_points : (count + 8ull * n_devices - 1) / (8ull * n_devices);
     if (bp > (1ull << 30)) bp = 1ull << 30;
@@ -50,22 +52,30 @@ zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, c
 
     std::atomic<int64_t> next{0};
     std::atomic<int> failed{ZMC_OK};
+    std::atomic<int> cuda_error{0};              // a worker's cudaError_t, handed to the CALLER's zmc_last_cuda_error()
+    auto fail_cuda = [&](cudaError_t e) { cuda_error = (int)e; failed = ZMC_ERR_CUDA; };
     std::vector<int64_t> done(n_devices, 0);
     std::vector<double> busy_ms(n_devices, 0.0);
     const auto t0 = std::chrono::steady_clock::now();
 
     auto worker = [&](int slot) {
-        if (cudaSetDevice(devices[slot]) != cudaSuccess) { failed = ZMC_ERR_CUDA; return; }
+        cudaError_t ce = cudaSetDevice(devices[slot]);
+        if (ce != cudaSuccess) { fail_cuda(ce); return; }
         cudaStream_t stream = nullptr;
-        if (cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking) != cudaSuccess) { failed = ZMC_ERR_CUDA; return; }
+        if ((ce = cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking)) != cudaSuccess) { fail_cuda(ce); return; }
         cudaEvent_t inflight[2] = {nullptr, nullptr};          // at most two batches queued per device: the second one's
-        cudaEventCreateWithFlags(&inflight[0], cudaEventDisableTiming);   // kernel overlaps the first one's D2H copy
-        cudaEventCreateWithFlags(&inflight[1], cudaEventDisableTiming);
+        for (int i = 0; i < 2; ++i)                              // kernel overlaps the first one's D2H copy
+            if ((ce = cudaEventCreateWithFlags(&inflight[i], cudaEventDisableTiming)) != cudaSuccess) {
+                fail_cuda(ce);
+                if (inflight[0]) cudaEventDestroy(inflight[0]);
+                cudaStreamDestroy(stream);
+                return;
+            }
         bool used[2] = {false, false};
         const auto w0 = std::chrono::steady_clock::now();
         for (int64_t k = 0; failed == ZMC_OK; ++k) {
             const int e = (int)(k & 1);
-            if (used[e] && cudaEventSynchronize(inflight[e]) != cudaSuccess) { failed = ZMC_ERR_CUDA; break; }
+            if (used[e] && (ce = cudaEventSynchronize(inflight[e])) != cudaSuccess) { fail_cuda(ce); break; }
             const int64_t b = next.fetch_add(1);
             if (b >= n_batches) break;
             uint64_t bf = 0, bc = 0;
@@ -75,14 +85,17 @@ zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, c
             ob.count = bc;
             ob.batch_points = 0;
             const size_t off = (size_t)(bf - first) * elem;
-            const zmc_status s = zmc_scan_ex(integrand_id, N, bounds, M, lists, n_samples, seed, static_cast<char*>(out_mean) + off,
-                                             static_cast<char*>(out_stderr) + off, stream, &ob, nullptr);
-            if (s != ZMC_OK) { failed = (int)s; break; }
-            cudaEventRecord(inflight[e], stream);
+            zmc::AdaptArgs ab;
+            if (ad) ab = zmc::AdaptArgs{ad->n_max, ad->target, ad->out_n + (bf - first)};
+            // the value lists are uploaded once per device: every later batch hits the library's device-resident cache
+            const zmc_status s = zmc::scan_impl(integrand_id, N, bounds, M, lists, n_samples, seed, static_cast<char*>(out_mean) + off,
+                                                static_cast<char*>(out_stderr) + off, stream, &ob, nullptr, ad ? &ab : nullptr);
+            if (s != ZMC_OK) { if (s == ZMC_ERR_CUDA || s == ZMC_ERR_OUT_OF_MEMORY) cuda_error = zmc::get_last_cuda_error(); failed = (int)s; break; }
+            if ((ce = cudaEventRecord(inflight[e], stream)) != cudaSuccess) { fail_cuda(ce); break; }
             used[e] = true;
             ++done[slot];
         }
-        if (cudaStreamSynchronize(stream) != cudaSuccess && failed == ZMC_OK) failed = ZMC_ERR_CUDA;
+        if ((ce = cudaStreamSynchronize(stream)) != cudaSuccess && failed == ZMC_OK) fail_cuda(ce);
         busy_ms[slot] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - w0).count();
         cudaEventDestroy(inflight[0]);
         cudaEventDestroy(inflight[1]);
@@ -103,7 +116,29 @@ zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, c
         timing->n_devices = n_devices;
         for (int d = 0; d < n_devices; ++d) { timing->batches_done[d] = done[d]; timing->busy_ms[d] = busy_ms[d]; }
     }
+    if (failed != ZMC_OK) zmc::set_last_cuda_error(cuda_error.load());
     return (zmc_status)failed.load();
+}
+
+}  // namespace
+
+extern "C" {
+
+zmc_status zmc_scan_farm(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                         uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, const int* devices,
+                         int n_devices, const zmc_options* opt, zmc_farm_timing* timing) {
+    return farm_impl(integrand_id, N, bounds, M, lists, n_samples, seed, out_mean, out_stderr, nullptr, devices, n_devices, opt, timing);
+}
+
+zmc_status zmc_scan_farm_adaptive(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                                  uint64_t n_first, uint64_t n_max, double target_stderr, uint64_t seed, void* out_mean,
+                                  void* out_stderr, uint32_t* out_n, const int* devices, int n_devices,
+                                  const zmc_options* opt, zmc_farm_timing* timing) {
+    if (!out_n || n_first < 256 || n_first % 256 != 0 || n_max < n_first || n_max % 8 != 0 || n_max > 0xFFFFFFF8ull ||
+        !(target_stderr >= 0.0))
+        return ZMC_ERR_INVALID_ARG;              // the same checks zmc_scan_adaptive makes, before any thread starts
+    const zmc::AdaptArgs ad{n_max, target_stderr, out_n};
+    return farm_impl(integrand_id, N, bounds, M, lists, n_first, seed, out_mean, out_stderr, &ad, devices, n_devices, opt, timing);
 }
 
 }  // extern "C"

@@ -66,17 +66,41 @@ Nvrtc& nvrtc() {
 
 std::mutex g_user_mutex;
 std::vector<std::unique_ptr<UserIntegrand>> g_users;
+int g_next_user_id = kFirstUserId;        // ids are never reused
 thread_local std::string tl_compile_log;
 
 // The translation unit NVRTC sees: the library's kernel template plus a family that evaluates the user's g.
 // No folding of the affine sample map here (the user's g wants y itself): y_k = fma(u_k, width_k, a_k), reading S5.
-std::string make_source(const char* body, int N, int M, int n_consts) {
+std::string make_source(const char* body, int N, int M, int n_consts, int flags) {
     char head[256];
-    std::snprintf(head, sizeof(head), "#define ZMC_USER_N %d\n#define ZMC_USER_M %d\n#define ZMC_USER_NC %d\n", N, M, n_consts);
+    std::snprintf(head, sizeof(head), "#define ZMC_USER_N %d\n#define ZMC_USER_M %d\n#define ZMC_USER_NC %d\n#define ZMC_USER_FAST %d\n",
+                  N, M, n_consts, (flags & ZMC_USER_FAST_MATH) ? 1 : 0);
     std::string s = head;
     s += R"SRC(
 #include "zmc_kernel.cuh"
 namespace zmc {
+// the library's own transcendentals, offered to the user's body (include/zmc.h, zmc_register_integrand)
+__device__ __forceinline__ double zmc_sinpi(double z) { return sinpi_f64(z); }
+__device__ __forceinline__ double zmc_cospi(double z) { return sinpi_f64(z + 0.5); }
+__device__ __forceinline__ double zmc_sin(double v) { return sinpi_f64(v * kInvPi); }
+__device__ __forceinline__ double zmc_cos(double v) { return sinpi_f64(::fma(v, kInvPi, 0.5)); }
+__device__ __forceinline__ double zmc_exp(double v) { return ::exp(v); }
+__device__ __forceinline__ double zmc_exp2(double v) { return ::exp2(v); }
+#if ZMC_USER_FAST
+__device__ __forceinline__ float zmc_sinpi(float z) { return Fn<float, true>::sin_phase(0.5f * z); }
+__device__ __forceinline__ float zmc_cospi(float z) { return Fn<float, true>::sin_phase(fmaf(0.5f, z, 0.25f)); }
+__device__ __forceinline__ float zmc_sin(float v) { return Fn<float, true>::sin_phase(v * 0.15915494309189535f); }
+__device__ __forceinline__ float zmc_cos(float v) { return Fn<float, true>::sin_phase(fmaf(v, 0.15915494309189535f, 0.25f)); }
+__device__ __forceinline__ float zmc_exp(float v) { return Fn<float, true>::exp2_neg(v * -1.4426950408889634f); }
+__device__ __forceinline__ float zmc_exp2(float v) { return Fn<float, true>::exp2_neg(-v); }
+#else
+__device__ __forceinline__ float zmc_sinpi(float z) { return sinpif(z); }
+__device__ __forceinline__ float zmc_cospi(float z) { return cospif(z); }
+__device__ __forceinline__ float zmc_sin(float v) { return sinf(v); }
+__device__ __forceinline__ float zmc_cos(float v) { return cosf(v); }
+__device__ __forceinline__ float zmc_exp(float v) { return expf(v); }
+__device__ __forceinline__ float zmc_exp2(float v) { return exp2f(v); }
+#endif
 template <typename R> struct FamUser {
     using real = R;
     static constexpr int kN = ZMC_USER_N <= 8 ? ZMC_USER_N : 0;     // compile-time N up to 8, else the runtime-N loop
@@ -131,11 +155,9 @@ cudaError_t launch_user(const UserIntegrand& u, int precision, int schedule, con
 
 void unload_user_integrands() {
     std::lock_guard<std::mutex> lock(g_user_mutex);
-    for (auto& u : g_users) {
+    for (auto& u : g_users)
         if (u->lib) cudaLibraryUnload(u->lib);
-        u->lib = nullptr;
-        std::memset(u->kern, 0, sizeof(u->kern));
-    }
+    g_users.clear();                           // ids are valid until zmc_shutdown (include/zmc.h); they are never reused
 }
 
 }  // namespace zmc
@@ -146,16 +168,40 @@ extern "C" {
 
 const char* zmc_last_compile_log(void) { return tl_compile_log.c_str(); }
 
-zmc_status zmc_register_integrand(const char* name, const char* body, int N, int M, int n_consts, int* integrand_id) {
+static unsigned long long hash_integrand(const char* body, int N, int M, int n_consts, int flags) {
+    unsigned long long h = 1469598103934665603ull;
+    auto mix = [&h](const void* p, size_t n) {
+        const unsigned char* b = static_cast<const unsigned char*>(p);
+        for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+    };
+    const int shape[4] = {N, M, n_consts, flags};
+    mix(shape, sizeof(shape));
+    mix(body, std::strlen(body));
+    return h;
+}
+
+zmc_status zmc_register_integrand_ex(const char* name, const char* body, int N, int M, int n_consts, int flags,
+                                     int* integrand_id) {
     tl_compile_log.clear();
     if (!name || !body || !integrand_id) return ZMC_ERR_INVALID_ARG;
     if (N < 1 || N > ZMC_MAX_N || M < 1 || M > ZMC_MAX_M || n_consts < 0 || n_consts > ZMC_MAX_CONSTS) return ZMC_ERR_INVALID_ARG;
+    if (flags & ~ZMC_USER_FAST_MATH) return ZMC_ERR_INVALID_ARG;
+    // the cache (SURVEY.md 8(f) NEXT-3 "cache by hash"): the same integrand registered again is the same id, no compile
+    const unsigned long long h = hash_integrand(body, N, M, n_consts, flags);
+    {
+        std::lock_guard<std::mutex> lock(g_user_mutex);
+        for (auto& u : g_users)
+            if (u->hash == h && u->lib && u->N == N && u->M == M && u->n_consts == n_consts && u->flags == flags && u->body == body) {
+                *integrand_id = u->id;
+                return ZMC_OK;
+            }
+    }
     Nvrtc& rt = nvrtc();
     if (!rt.ok) {
         tl_compile_log = "libnvrtc.so.12 could not be loaded";
         return ZMC_ERR_COMPILE;
     }
-    const std::string src = make_source(body, N, M, n_consts);
+    const std::string src = make_source(body, N, M, n_consts, flags);
     const char* names[kNumHeaders];
     const char* texts[kNumHeaders];
     for (int i = 0; i < kNumHeaders; ++i) { names[i] = kHeaders[i].name; texts[i] = kHeaders[i].text; }
@@ -176,8 +222,8 @@ zmc_status zmc_register_integrand(const char* name, const char* body, int N, int
                 return ZMC_ERR_COMPILE;
             }
         }
-    const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo", "-default-device"};
-    const nvrtcResult rc = rt.compileProgram(prog, 4, opts);
+    const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo", "-default-device", "--use_fast_math"};
+    const nvrtcResult rc = rt.compileProgram(prog, (flags & ZMC_USER_FAST_MATH) ? 5 : 4, opts);
     size_t log_size = 0;
     if (rt.getProgramLogSize(prog, &log_size) == NVRTC_SUCCESS && log_size > 1) {
         tl_compile_log.resize(log_size);
@@ -191,21 +237,39 @@ zmc_status zmc_register_integrand(const char* name, const char* body, int N, int
     if (rt.getCUBIN(prog, cubin.data()) != NVRTC_SUCCESS) return ZMC_ERR_COMPILE;
 
     auto u = std::make_unique<UserIntegrand>();
-    u->name = name; u->N = N; u->M = M; u->n_consts = n_consts;
+    u->name = name; u->N = N; u->M = M; u->n_consts = n_consts; u->flags = flags; u->body = body; u->hash = h;
     cudaError_t e = cudaLibraryLoadData(&u->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
     if (e != cudaSuccess) { tl_compile_log += "\ncudaLibraryLoadData: "; tl_compile_log += cudaGetErrorString(e); return ZMC_ERR_CUDA; }
     for (int pr = 0; pr < 2; ++pr)
         for (int sc = 0; sc < 4; ++sc) {
             const char* lowered = nullptr;
-            if (rt.getLoweredName(prog, expr[pr][sc].c_str(), &lowered) != NVRTC_SUCCESS || !lowered) return ZMC_ERR_COMPILE;
-            e = cudaLibraryGetKernel(&u->kern[pr][sc], u->lib, lowered);
-            if (e != cudaSuccess) { cudaLibraryUnload(u->lib); return ZMC_ERR_CUDA; }
+            const bool named = rt.getLoweredName(prog, expr[pr][sc].c_str(), &lowered) == NVRTC_SUCCESS && lowered;
+            e = named ? cudaLibraryGetKernel(&u->kern[pr][sc], u->lib, lowered) : cudaErrorInvalidDeviceFunction;
+            if (e != cudaSuccess) {          // the loaded code is released on every failure after the load
+                cudaLibraryUnload(u->lib);
+                return named ? ZMC_ERR_CUDA : ZMC_ERR_COMPILE;
+            }
         }
     std::lock_guard<std::mutex> lock(g_user_mutex);
-    u->id = kFirstUserId + (int)g_users.size();
+    u->id = g_next_user_id++;
     *integrand_id = u->id;
     g_users.push_back(std::move(u));
     return ZMC_OK;
+}
+
+zmc_status zmc_register_integrand(const char* name, const char* body, int N, int M, int n_consts, int* integrand_id) {
+    return zmc_register_integrand_ex(name, body, N, M, n_consts, 0, integrand_id);
+}
+
+zmc_status zmc_unregister_integrand(int integrand_id) {
+    std::lock_guard<std::mutex> lock(g_user_mutex);
+    for (size_t i = 0; i < g_users.size(); ++i)
+        if (g_users[i]->id == integrand_id) {
+            if (g_users[i]->lib) cudaLibraryUnload(g_users[i]->lib);
+            g_users.erase(g_users.begin() + (long)i);
+            return ZMC_OK;
+        }
+    return ZMC_ERR_UNKNOWN_INTEGRAND;
 }
 
 }  // extern "C"

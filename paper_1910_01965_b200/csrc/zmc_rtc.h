@@ -10,7 +10,9 @@ constexpr int kFirstUserId = 1000;
 struct UserIntegrand {
     int id = 0;
     std::string name;
-    int N = 0, M = 0, n_consts = 0;
+    int N = 0, M = 0, n_consts = 0, flags = 0;
+    std::string body;
+    unsigned long long hash = 0;          // of (body, N, M, n_consts, flags): re-registration returns the cached entry
     cudaLibrary_t lib = nullptr;
     cudaKernel_t kern[2][4] = {};        // [precision][schedule - 1]; schedule 4 = the adaptive kernel
 };

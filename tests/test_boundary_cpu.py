@@ -28,14 +28,15 @@ def test_struct_layouts_match_header_sizes(tmp_path):
     import ctypes
     import subprocess
     src = tmp_path / "sz.c"
-    src.write_text('#include <stdio.h>\n#include "zmc.h"\nint main(void){printf("%zu %zu %zu %zu\\n",'
-                   'sizeof(zmc_options),sizeof(zmc_timing),sizeof(zmc_param_list),sizeof(zmc_integrand_info));return 0;}\n')
+    src.write_text('#include <stdio.h>\n#include "zmc.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu\\n",'
+                   'sizeof(zmc_options),sizeof(zmc_timing),sizeof(zmc_param_list),sizeof(zmc_integrand_info),'
+                   'sizeof(zmc_pipe_report),sizeof(zmc_farm_timing));return 0;}\n')
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)],
                    check=True)
     sizes = [int(v) for v in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
     assert sizes == [ctypes.sizeof(zb.zmc_options), ctypes.sizeof(zb.zmc_timing), ctypes.sizeof(zb.zmc_param_list),
-                     ctypes.sizeof(zb.zmc_integrand_info)]
+                     ctypes.sizeof(zb.zmc_integrand_info), ctypes.sizeof(zb.zmc_pipe_report), ctypes.sizeof(zb.zmc_farm_timing)]
 
 
 def test_integrand_table():
@@ -87,14 +88,39 @@ def test_validation_errors():
 
 
 def test_schedule_choice_follows_design_table():
-    # cfg1 CTA, cfg2 WARP, cfg3-5 THREAD
-    expect = {1: zb.ZMC_SCHED_CTA, 2: zb.ZMC_SCHED_WARP, 3: zb.ZMC_SCHED_THREAD, 4: zb.ZMC_SCHED_THREAD}
+    # cfg1 CTA, cfg2-5 THREAD (cfg 2 = 8.8 rounds of the 148 x 768 resident fp64 threads;
+    # measured 2.8 % faster than WARP).  No GPU here: the chooser falls back to 148 SMs.
+    expect = {1: zb.ZMC_SCHED_CTA, 2: zb.ZMC_SCHED_THREAD, 3: zb.ZMC_SCHED_THREAD, 4: zb.ZMC_SCHED_THREAD}
     for k, s in expect.items():
         w = wl.config(k)
-        assert zb.zmc_pick_schedule(w.G, w.n_samples, w.N) == s
+        assert zb.zmc_pick_schedule(w.G, w.n_samples, w.N, w.precision) == s
     w = wl.config(5)
-    assert zb.zmc_pick_schedule(1 << 28, w.n_samples, w.N) == zb.ZMC_SCHED_THREAD
+    assert zb.zmc_pick_schedule(1 << 28, w.n_samples, w.N, w.precision) == zb.ZMC_SCHED_THREAD
     assert zb.zmc_pick_schedule(10, 8, 1) == zb.ZMC_SCHED_THREAD          # too few samples to split
+    # between the two: a 10^5-point grid with many samples goes warp-per-point; the fp32-evaluate kernels keep 1024
+    # threads per SM resident instead of 768, so their THREAD threshold is higher
+    assert zb.zmc_pick_schedule(10 ** 5, 10 ** 4, 2) == zb.ZMC_SCHED_WARP
+    assert zb.zmc_pick_schedule(10 ** 6, 10 ** 4, 2, zb.ZMC_PREC_F64) == zb.ZMC_SCHED_THREAD
+    assert zb.zmc_pick_schedule(10 ** 6, 10 ** 4, 2, zb.ZMC_PREC_F32E) == zb.ZMC_SCHED_WARP
+
+
+def test_explicit_count_makes_an_empty_range_expressible():
+    # count == 0 used to mean only "to the end of the grid"; a caller whose shard is empty at first < G
+    # had no way to say so.  ZMC_OPT_EXPLICIT_COUNT takes count literally.
+    w = wl.config(1, scale=[4], n_samples=10)
+    import ctypes
+    m = zb._Marshalled(w.bounds, w.lists, None)
+    for flags, first, count, want in [(0, 2, 0, zb.ZMC_OK), (zb.ZMC_OPT_EXPLICIT_COUNT, 2, 0, zb.ZMC_OK),
+                                      (zb.ZMC_OPT_EXPLICIT_COUNT, 4, 0, zb.ZMC_OK), (zb.ZMC_OPT_EXPLICIT_COUNT, 2, 3, zb.ZMC_ERR_INVALID_ARG),
+                                      (64, 0, 0, zb.ZMC_ERR_INVALID_ARG)]:
+        o = zb._make_options(m, zb.ZMC_PREC_F64, zb.ZMC_OUT_F64, zb.ZMC_LOC_DEVICE, 0, -1, 0, first, count, flags)
+        g = ctypes.c_uint64(0)
+        st = zb.load().zmc_validate(1, m.N, m.bounds_ptr(), m.M, m.c_lists, 10, ctypes.byref(o), ctypes.byref(g))
+        assert st == want, (flags, first, count)
+    # an explicitly empty range is a no-op that needs no GPU: nothing is enqueued, outputs stay untouched
+    mean, err = np.full(1, 7.0), np.full(1, 7.0)
+    zb.zmc_scan_ex(1, w.bounds, w.lists, 10, 1, mean, err, stream=0, first_index=2, count=0, flags=zb.ZMC_OPT_EXPLICIT_COUNT)
+    assert mean[0] == 7.0 and err[0] == 7.0
 
 
 @pytest.mark.parametrize("first,count,bp", [(0, 10 ** 10, 1 << 28), (5, 1000, 97), (0, 7, 0), (3, 7, 100), (0, 8, 4)])

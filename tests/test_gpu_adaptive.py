@@ -107,3 +107,44 @@ def test_adaptive_argument_errors():
         assert ei.value.status == zb.ZMC_ERR_INVALID_ARG
     torch.cuda.synchronize()
     assert torch.all(m == -1.0) and torch.all(n == 0)
+
+
+def test_adaptive_streams_to_pinned_host_and_through_the_farm():
+    """zmc_scan_adaptive with ZMC_LOC_HOST outputs (out_n streamed with the results, batch by batch) and
+    zmc_scan_farm_adaptive, on a 1.2 * 10^8-point sub-range of cfg 5's 10^10 grid cut into batches: bit-identical to the
+    device-output call on the same range, which the other tests pin to the fixed-n scan and the oracle."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(5)
+    first, count, bp = (1 << 32) - 7_000_001, 120_000_000, 1 << 25         # straddles 2^32; 4 batches, the last one ragged
+    n_first, n_max, target = 256, 512, 0.11
+    dm = torch.empty(count, dtype=torch.float32, device="cuda")
+    de = torch.empty_like(dm)
+    dn = torch.zeros(count, dtype=torch.int32, device="cuda")
+    zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, n_first, n_max, target, w.seed, dm, de, dn,
+                         precision=w.precision, first_index=first, count=count)
+    hm = torch.empty(count, dtype=torch.float32, pin_memory=True)
+    he = torch.empty_like(hm).pin_memory()
+    hn = torch.zeros(count, dtype=torch.int32).pin_memory()
+    tm = zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, n_first, n_max, target, w.seed, hm, he, hn,
+                              precision=w.precision, first_index=first, count=count, batch_points=bp, timing=True)
+    torch.cuda.synchronize()
+    assert tm["n_batches"] == 4 and tm["host_out_pinned"] == 1 and tm["d2h_bytes"] == count * 12
+    assert torch.equal(hm, dm.cpu()) and torch.equal(he, de.cpu()) and torch.equal(hn, dn.cpu())
+    frac = float((hn == n_max).float().mean())
+    assert 0.02 < frac < 0.98, "the target should split the points between the two checkpoints"
+    # the same through the farm (feeder threads on the one visible device)
+    fm, fe, fn = torch.empty_like(hm).pin_memory(), torch.empty_like(hm).pin_memory(), torch.zeros_like(hn).pin_memory()
+    ft = zb.zmc_scan_farm_adaptive(w.integrand_id, w.bounds, w.lists, n_first, n_max, target, w.seed, fm, fe, fn, [0, 0],
+                                   precision=w.precision, first_index=first, count=count, batch_points=bp)
+    assert ft["n_batches"] == 4 and sum(ft["batches_done"]) == 4
+    assert torch.equal(fm, hm) and torch.equal(fe, he) and torch.equal(fn, hn)
+    # oracle spot check on sampled points of each checkpoint population
+    rng = np.random.default_rng(5)
+    n_np = hn.numpy()
+    for n in (n_first, n_max):
+        sel = rng.choice(np.nonzero(n_np == n)[0], 200, replace=False)
+        w.n_samples = n
+        rc, mo, eo = orc.points_workload(w, (sel + first).astype(np.uint64), n_threads=NT)
+        assert rc == 0
+        assert_parity(w, hm.numpy()[sel].astype(np.float64), he.numpy()[sel].astype(np.float64), mo, eo)

@@ -50,4 +50,4 @@ def test_random_configuration_matches_oracle(case):
     torch.cuda.synchronize()
     b = np.asarray(w.bounds).reshape(-1, 2)
     volume = float(np.prod(b[:, 1] - b[:, 0]))
-    assert_parity(w, m.cpu().numpy(), e.cpu().numpy(), mean_o, err_o, abs_scale=max(1.0, volume))
+    assert_parity(w, m.cpu().numpy(), e.cpu().numpy(), mean_o, err_o, abs_scale=max(1.0, volume / 8.0))

@@ -25,11 +25,15 @@ def _zb():
     return binding
 
 
-def assert_parity(w, mean, err, mean_o, err_o, abs_scale=1.0):
+def assert_parity(w, mean, err, mean_o, err_o, abs_scale=1.0, eps_g=0.0):
+    """eps_g: the per-sample disagreement |g_gpu - g_oracle| the two evaluations of g may have (DESIGN.md section 2,
+    "nearly constant integrands"): it moves the stderr by at most V eps_g / sqrt(n-1) whatever the spread of g is."""
     mean, err = np.asarray(mean, dtype=np.float64), np.asarray(err, dtype=np.float64)
     if w.precision == wl.PREC_F64 and not w.out_f32:
+        b = np.asarray(w.bounds).reshape(-1, 2)
+        floor = float(np.prod(b[:, 1] - b[:, 0])) * eps_g / np.sqrt(w.n_samples - 1.0)
         tol_m = 1e-10 * np.maximum(np.abs(mean_o), err_o)
-        tol_e = 1e-10 * err_o
+        tol_e = 1e-10 * err_o + floor
         bad_m = np.abs(mean - mean_o) > tol_m + 1e-300
         bad_e = np.abs(err - err_o) > tol_e + 1e-300
     else:
@@ -142,15 +146,25 @@ def test_indices_above_2_pow_32():
 
 
 def test_nearly_constant_integrand_stderr():
-    # hard part 3 of SURVEY.md section 7: raw sums lose the stderr of a nearly constant integrand
-    # (2.6e-9 at x1 = 0.1).  Below x1 ~ 0.01 the spread of g drops under 1e-5 |g| and the last-ulp
-    # difference between libm cos and the kernel's polynomial alone exceeds 1e-10 of the stderr.
+    # hard part 3 of SURVEY.md section 7: raw sums lose the stderr of a nearly constant integrand (2.6e-9 at x1 = 0.1);
+    # the shifted sums keep it.  For x1 >= 0.01 the plain 1e-10 tolerance holds.
     w = wl.config(1, scale=[5], n_samples=10_000)
     w.lists = [np.array([0.01, 0.02, 0.05, 0.1, 0.3])]
     rc, mean_o, err_o = orc.scan_workload(w)
     for sched in (1, 2, 3):
         mean, err = run_gpu(w, schedule=sched)
         assert_parity(w, mean, err, mean_o, err_o)
+    # Below x1 ~ 5e-3 the spread of g = cos(x1 y) (0.149 x1^2) falls under 4e-6 and the last-bit difference between
+    # libm's cos (the oracle, <= 1 ulp = 2.2e-16 near 1) and the kernel's own polynomial (<= 2.4e-16) is no longer
+    # 1e-10 of it.  DESIGN.md section 2 states the limit: |d stderr| <= 1e-10 stderr_o + V eps_g / sqrt(n-1) with
+    # eps_g = 4.6e-16 the two evaluations' combined worst case (a rigorous bound: perturbing every g_s by <= eps_g moves
+    # ||g - mean(g)|| by <= eps_g sqrt(n)).  These are the points the round-1 test dropped; the mean keeps the plain bound.
+    w.lists = [np.array([1e-4, 3e-4, 1e-3, 3e-3])]
+    rc, mean_o, err_o = orc.scan_workload(w)
+    assert np.all(err_o > 0)
+    for sched in (1, 2, 3):
+        mean, err = run_gpu(w, schedule=sched)
+        assert_parity(w, mean, err, mean_o, err_o, eps_g=4.6e-16)
 
 
 def test_stream_ordering_and_default_entry_point():
@@ -187,7 +201,42 @@ def test_timing_struct():
     zb = _zb()
     w = wl.config(5, scale=[6, 6, 6, 6, 6], n_samples=64)
     w.batch_points = 2000
-    m, e, tm = zb.scan_workload(w, timing=True)
-    assert tm["n_batches"] == 4 and tm["gpu_launches"] == 4
+    m, e, tm = zb.scan_workload(w, timing=True, flags=zb.ZMC_OPT_FRESH_LISTS)
+    assert tm["n_batches"] == 4 and tm["gpu_launches"] == 4 and tm["host_out_pinned"] == 1
     assert tm["d2h_bytes"] == 2 * 4 * w.G and tm["h2d_bytes"] == 8 * 30
     assert tm["kernel_ms"] > 0 and tm["wall_ms"] >= tm["kernel_ms"] * 0.99 and tm["d2h_ms"] > 0
+
+
+def test_value_lists_are_cached_on_the_device_by_content():
+    """H1: a repeated call with the same lists copies nothing (h2d_bytes == 0); different values in lists of the same
+    shape are a different cache entry (and give different results); ZMC_OPT_FRESH_LISTS forces the upload; the cache
+    survives more distinct list sets than it has slots (eviction) and use from a second stream."""
+    import torch
+    zb = _zb()
+    w = wl.config(2, scale=[17, 13], n_samples=300)
+    w.lists[0] = w.lists[0] + 0.001234            # values no other test uses
+    rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
+    m, e, t1 = zb.scan_workload(w, timing=True)
+    m2, e2, t2 = zb.scan_workload(w, timing=True)
+    m3, e3, t3 = zb.scan_workload(w, timing=True, flags=zb.ZMC_OPT_FRESH_LISTS)
+    torch.cuda.synchronize()
+    assert t1["h2d_bytes"] == 8 * 30 and t2["h2d_bytes"] == 0 and t3["h2d_bytes"] == 8 * 30
+    assert torch.equal(m, m2) and torch.equal(m, m3) and torch.equal(e, e3)
+    assert_parity(w, m.cpu().numpy(), e.cpu().numpy(), mean_o, err_o)
+    w2 = wl.config(2, scale=[17, 13], n_samples=300)
+    w2.lists[0] = w.lists[0].copy()
+    w2.lists[1] = w.lists[1] * 1.0000001          # same shape, one list differs in the last digits
+    rc, mean_o2, err_o2 = orc.scan_workload(w2, n_threads=NT)
+    mb, eb, tb = zb.scan_workload(w2, timing=True)
+    torch.cuda.synchronize()
+    assert tb["h2d_bytes"] == 8 * 30 and not torch.equal(mb, m)
+    assert_parity(w2, mb.cpu().numpy(), eb.cpu().numpy(), mean_o2, err_o2)
+    # more list sets than cache slots, from two streams; the first set must still give the first result afterwards
+    side = torch.cuda.Stream()
+    for k in range(12):
+        wk = wl.config(2, scale=[17, 13], n_samples=300)
+        wk.lists[0] = w.lists[0] + 0.01 * (k + 1)
+        zb.scan_workload(wk, stream=side if k % 2 else None)
+    m4, e4, t4 = zb.scan_workload(w, timing=True, stream=side)
+    torch.cuda.synchronize()
+    assert t4["h2d_bytes"] == 8 * 30 and torch.equal(m4, m) and torch.equal(e4, e)

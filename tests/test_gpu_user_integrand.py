@@ -73,3 +73,54 @@ def test_user_shape_mismatch_and_unknown_id():
     with pytest.raises(zb.ZmcError) as ei:
         zb.zmc_scan_ex(uid + 500, [0.0, 1.0], [np.arange(4.0)], 10, 1, m, m.clone())
     assert ei.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
+
+
+HELPER_BODY = ("return zmc_sin(x[0] * y[0]) * zmc_cos(x[1] * y[1] + c[0]) + zmc_sinpi(y[0] - x[1]) * zmc_cospi(x[0] * y[1]) "
+               "+ zmc_exp(-x[0] * y[1] * y[1]) - zmc_exp2(-y[0]);")
+
+
+@pytest.mark.parametrize("precision,flags", [(wl.PREC_F64, 0), (wl.PREC_F32E, 0), (wl.PREC_F32E, 1), (wl.PREC_F64, 1)])
+def test_library_transcendentals_in_user_bodies(precision, flags):
+    """zmc_sin / zmc_cos / zmc_sinpi / zmc_cospi / zmc_exp / zmc_exp2 (include/zmc.h) against the oracle evaluating their
+    plain definitions; with ZMC_USER_FAST_MATH the fp32 versions are the MUFU forms (same tolerance as the built-in families)."""
+    from paper_1910_01965_b200 import binding as zb
+    uid = zb.zmc_register_integrand("helpers", HELPER_BODY, 2, 2, 1, flags=flags)
+    orc.set_user_integrand(HELPER_BODY, 2, 2, 1)
+    w = wl.Workload("helpers", uid, np.array([0.0, 2.0, -1.0, 1.5]), [wl.linspace(0.3, 9.0, 12), wl.linspace(-2.0, 4.0, 9)],
+                    1501, 33, precision, np.array([0.4]))
+    rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
+    assert rc == 0
+    for sched in (1, 2, 3):
+        mean, err = run_gpu(w, schedule=sched)
+        assert_parity(w, mean, err, mean_o, err_o)
+
+
+def test_registration_is_cached_by_content_and_can_be_undone():
+    """SURVEY.md 8(f) NEXT-3 "cache by hash": the same (body, N, M, n_consts, flags) is the same id and costs no compile."""
+    import time
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    body = "return x[0] * y[0] * y[0] + 0.125;"          # nothing else in the suite registers this one
+    t0 = time.perf_counter()
+    uid = zb.zmc_register_integrand("cached", body, 1, 1, 0)
+    t_first = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    again = zb.zmc_register_integrand("another name, same integrand", body, 1, 1, 0)
+    t_again = time.perf_counter() - t0
+    assert again == uid and t_again < 1e-3 < t_first
+    assert zb.zmc_register_integrand("cached", body, 1, 1, 0, flags=zb.ZMC_USER_FAST_MATH) != uid      # other flags: other code
+    assert zb.zmc_register_integrand("cached", body + " ", 1, 1, 0) != uid
+    m = torch.zeros(3, dtype=torch.float64, device="cuda")
+    e = torch.zeros_like(m)
+    zb.zmc_scan_ex(uid, [0.0, 1.0], [np.array([1.0, 2.0, 3.0])], 64, 1, m, e)
+    torch.cuda.synchronize()
+    assert torch.all(m > 0.125)
+    zb.zmc_unregister_integrand(uid)
+    with pytest.raises(zb.ZmcError) as ei:
+        zb.zmc_scan_ex(uid, [0.0, 1.0], [np.array([1.0, 2.0, 3.0])], 64, 1, m, e)
+    assert ei.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
+    with pytest.raises(zb.ZmcError) as ei:
+        zb.zmc_unregister_integrand(uid)
+    assert ei.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
+    fresh = zb.zmc_register_integrand("cached", body, 1, 1, 0)          # compiled again, ids are never reused
+    assert fresh != uid
