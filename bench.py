@@ -1,16 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the zmc_scan hot path on B200 (driver contract in the task prompt).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl reference]
 
-A "step" is one pass of the whole hot path (H1-H8: stage lists, decode, Philox, integrand, fp64
-reduce, finalise, store) over one synthetic workload of BASELINE.json `configs` (default
-configs[1] = cfg2; cfg5 streams its 80 GB of results to pinned host memory).  `value` is
-integrand evaluations/s with device-resident outputs; `e2e` is the same metric through the C ABI
-with HOST output buffers (list H2D and result D2H inside the timed region).  `roofline` is the
-measured-dispatch-cost ALU bound of DESIGN.md section 6 ("bound": "alu"); `cpu_baseline` is the CPU oracle, as it
-stands, on a bounded sample of the same workload.  With N > 1 (torchrun) the grid's first list is
-lengthened N-fold and each rank scans its own contiguous flat range -- no data-path collective.
+A "step" is one pass of the whole hot path (H1-H8: stage lists, decode, Philox, integrand, fp64 reduce, finalise,
+store) over one synthetic workload of BASELINE.json `configs`.  The default workload is cfg5, the largest
+single-GPU configuration (10^10 grid points x 256 samples): `value` is integrand
+evaluations/s with the 80 GB of results device-resident, `e2e` the same scan through the C ABI with pinned HOST
+outputs (list H2D forced, result D2H streamed in 2^28-point batches, `exposed_d2h_ms` = what compute did not hide).
+`per_config` carries the same record for cfg1-cfg4 (the north_star target is on cfg2-cfg4), `pipe_rates` the
+dispatch costs measured in this very run (zmc_measure_pipes) that the ALU roofline is built from, `cpu_baseline`
+the unoptimised CPU oracle on a bounded slice.  With N > 1 (torchrun) the grid's first list is lengthened N-fold and
+each rank scans its own contiguous flat range -- no data-path collective.
 """
 from __future__ import annotations
 
@@ -32,14 +33,13 @@ from paper_1910_01965_b200 import workloads as wl  # noqa: E402
 METRIC = "integrand_evals_per_s"
 UNIT = "evals/s"
 
-# ALU roofline.  The loop is bound by the SM sub-partition's dispatch of half-width (16-lane)
-# pipes, measured by `python -m paper_1910_01965_b200.pipe_rates` (profiles/r01_pipe_rates.txt): every integer
-# instruction (IMAD.WIDE, LOP3, SHF, IADD3) costs 2 SMSP-cycles per warp, every FP32 instruction 1, and the two
-# classes serialise on one port ("main"); FP64 instructions cost 2 on their own pipe, MUFU and F2F 8 each on the XU pipe.
-# W_MIN[cfg] = max over those resources of the ALGORITHMIC instruction list of one evaluation (Philox4x32-10 with the
-# t-only rounds hoisted = 16 IMAD.WIDE + 18 LOP3 per block, one bit-op per uniform (two for fp64), one FMA per
-# dimension, the integrand's own arithmetic, F2F + 2 fp64 accumulate ops), in SMSP-cycles per warp = lane-cycles per
-# thread.  (integer, FP32, FP64, XU) instructions per evaluation:
+# ALU roofline.  The loop is bound by the SM sub-partition's dispatch: every integer instruction
+# (IMAD.WIDE, LOP3, SHF, IADD3) costs 2 SMSP-cycles per warp, every FP32 instruction 1, and the two classes serialise
+# on one port ("main"); FP64 instructions cost 2 on their own pipe, MUFU and F2F 8 each on the XU pipe (`pipe_rates`
+# in the output re-measures these on every run).  W_MIN[cfg] = max over those resources of the ALGORITHMIC instruction
+# list of one evaluation (Philox4x32-10 with the t-only rounds hoisted = 16 IMAD.WIDE + 18 LOP3 per block, one bit-op
+# per uniform (two for fp64), one FMA per dimension, the integrand's own arithmetic, F2F + 2 fp64 accumulate ops), in
+# SMSP-cycles per warp = lane-cycles per thread.  (integer, FP32, FP64, XU) instructions per evaluation:
 ALG_OPS = {
     "cfg1": (0.25 * 34 + 2 + 2, 0, 1 + 12 + 2, 0),        # fp64 sinpi(z) - K: 12 fp64 + 2 integer (sign); phase FMA; 2 accumulate
     "cfg2": (0.50 * 34 + 4 + 2, 0, 2 + 12 + 2, 0),
@@ -52,17 +52,22 @@ ALG_OPS = {
 # 10^8 grid points x 10^5 samples; its V100 "GPU evaluation time per batch" 18.19497 s = 5.50e9 evals/s is the one
 # published number for exactly this workload, hence the one non-null vs_baseline.
 ALG_OPS["cfg2_user"] = ALG_OPS["cfg2"]     # same method, same minimum; the generic user path executes more
+ALG_OPS["cfg2_user_libdevice"] = ALG_OPS["cfg2"]
 SCAN_POINTS = {"eq4": 10**6}
 # NEXT-3: the cfg2 inputs with the integrand handed over as a user body and compiled with NVRTC at run time
-USER_BODIES = {"cfg2_user": ("cfg2", "return sin(x[0] * y[0] + x[1] * y[1]);")}
+USER_BODIES = {"cfg2_user": ("cfg2", "return zmc_sin(x[0] * y[0] + x[1] * y[1]);"),
+               "cfg2_user_libdevice": ("cfg2", "return sin(x[0] * y[0] + x[1] * y[1]);")}
 PUBLISHED_EVALS_PER_S = {"eq4": 1e6 * 1e5 / 18.19497}
+PER_CONFIG = ["cfg1", "cfg2", "cfg3", "cfg4"]
 
 
 def w_min(name):
     i, f, d, xu = ALG_OPS[name]
     res = {"main(int*2+fp32)": 2 * i + f, "fp64": 2 * d, "xu": 8 * xu, "issue": i + f + d + xu}
     bound = max(res, key=res.get)
-    return res[bound], bound, res
+    # what the same list costs if FP64 / XU instructions do NOT hide behind the integer stream but take one dispatch
+    # cycle each (what zmc_measure_pipes' "same warp" rows and every kernel of this library show on sm_100)
+    return res[bound], bound, res, 2 * i + f + d + xu
 
 
 SM_COUNT, LANES_PER_SM_CLK, SM_MAX_MHZ = 148, 128, 1965.0
@@ -79,6 +84,15 @@ def build_workload(name: str, world: int):
     return w
 
 
+def config_of(w, world: int):
+    """The `config` object: the workload, identical for the zmc arm and the reference arm."""
+    G_scan = SCAN_POINTS.get(w.name, w.G) * (world if w.name in SCAN_POINTS else 1)
+    return {"workload": w.name, "grid_points": w.G, "scanned_points": G_scan, "n_samples": w.n_samples, "N": w.N, "M": w.M,
+            "evals": G_scan * w.n_samples, "precision": "f64" if w.precision == wl.PREC_F64 else "f32 evaluate / f64 accumulate",
+            "out_dtype": "f32" if w.out_f32 else "f64", "seed": w.seed, "schedule": "auto",
+            "l2_flush_between_steps": True, "parallelism": f"index-range shards x{world}, no collective"}
+
+
 class ClockSampler:
     """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
@@ -93,6 +107,9 @@ class ClockSampler:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
                                           "-i", str(self.gpu), "-lms", "100"], stdout=subprocess.PIPE, text=True)
             threading.Thread(target=self._read, daemon=True).start()
+            t0 = time.time()                 # wait for the first sample: nvidia-smi's start-up (NVML initialisation) must
+            while not self.rows and time.time() - t0 < 3.0:      # not fall into a timed region that lasts milliseconds
+                time.sleep(0.01)
         except OSError:
             self.proc = None
 
@@ -115,45 +132,73 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
-def cpu_oracle_rate(w, seconds: float = 1.5):
-    """The oracle as it stands on all host cores, on a bounded contiguous slice from the middle of the grid."""
+def oracle_slice(w, n_threads: int, seconds: float, min_points: int):
+    """Time the CPU oracle, as it stands, on a contiguous slice from the middle of the grid: at least `min_points` grid
+    points and about `seconds` of work.  Returns (evals/s, seconds taken, points)."""
+    from oracle import zmc_oracle as orc
+    first = (w.G // 2 // 1000) * 1000
+    avail = w.G - first
+    probe = int(min(avail, max(n_threads * 4, 2e6 * n_threads / 16 // w.n_samples)))
+    t0 = time.perf_counter()
+    rc, _, _ = orc.scan_workload(w, first, probe, n_threads=n_threads)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    assert rc == 0
+    pts = int(min(avail, max(min_points, probe * seconds / dt)))
+    t0 = time.perf_counter()
+    rc, _, _ = orc.scan_workload(w, first, pts, n_threads=n_threads)
+    dt = time.perf_counter() - t0
+    assert rc == 0
+    return pts * w.n_samples / dt, dt, pts, first
+
+
+def cpu_baseline(w, seconds: float = 5.0, single_core: bool = True):
+    """BASELINE.md "CPU-baseline plan": the oracle on all host cores and on one core, each on a slice of
+    >= 10^5 grid points and >= `seconds` of work.  The oracle is deliberately plain (one Philox block per 32-bit word,
+    two-pass long-double estimator): a reported baseline, not a tuned CPU implementation -- no speed-up is claimed."""
     from oracle import zmc_oracle as orc
     if w.name in USER_BODIES:
         orc.set_user_integrand(USER_BODIES[w.name][1], w.N, w.M, len(w.consts))
         w.integrand_id = max(w.integrand_id, 1000)
     cores = os.cpu_count() or 1
-    first = (w.G // 2 // 1000) * 1000
-    probe = max(cores * 4, min(w.G - first, max(cores * 4, int(2e6 // w.n_samples))))
-    t0 = time.perf_counter()
-    rc, _, _ = orc.scan_workload(w, first, probe, n_threads=cores)
-    dt = max(time.perf_counter() - t0, 1e-4)
-    assert rc == 0
-    pts = int(min(w.G - first, max(probe, probe * seconds / dt)))
-    t0 = time.perf_counter()
-    rc, _, _ = orc.scan_workload(w, first, pts, n_threads=cores)
-    dt = time.perf_counter() - t0
-    assert rc == 0
-    return pts * w.n_samples / dt, cores, f"{pts} contiguous grid points from flat index {first} x {w.n_samples} samples"
+    min_pts = min(w.G // 2, 10 ** 5)
+    v, dt, pts, first = oracle_slice(w, cores, seconds, min_pts)
+    out = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle (unoptimised reference implementation)",
+           "sample": f"{pts} contiguous grid points from flat index {first} x {w.n_samples} samples", "seconds": dt}
+    if single_core:
+        v1, dt1, pts1, _ = oracle_slice(w, 1, seconds, max(1, min_pts // cores))
+        out["single_core"] = {"value": v1, "seconds": dt1, "points": pts1}
+    return out
 
 
 def run_reference(args, rank: int):
-    """--impl reference: the CPU oracle on the box's host cores (this tier has no reference code)."""
+    """--impl reference: the CPU oracle on the box's host cores (this tier has no reference code).  Each step is one
+    timed slice of the workload (>= 10^5 grid points, about 4 s of work); ms_per_step is that slice's real time."""
     if rank != 0:
         return
+    from oracle import zmc_oracle as orc
     w = build_workload(args.workload, 1)
-    vals = []
+    if w.name in USER_BODIES:
+        orc.set_user_integrand(USER_BODIES[w.name][1], w.N, w.M, len(w.consts))
+        w.integrand_id = max(w.integrand_id, 1000)
+    cores = os.cpu_count() or 1
+    vals, secs, sample = [], [], ""
+    budget = max(1.0, min(4.0, 150.0 / max(1, args.warmup + args.steps)))
     for i in range(args.warmup + args.steps):
-        v, cores, sample = cpu_oracle_rate(w, seconds=1.0)
+        v, dt, pts, first = oracle_slice(w, cores, budget, min(w.G // 2, 10 ** 5))
+        sample = f"{pts} contiguous grid points from flat index {first} x {w.n_samples} samples per step"
         if i >= args.warmup:
             vals.append(v)
+            secs.append(dt)
     value = float(np.mean(vals))
-    evals_per_step = value * 1.0
+    v1, dt1, pts1, _ = oracle_slice(w, 1, 3.0, max(1, min(w.G // 2, 10 ** 5) // cores))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * evals_per_step / value,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "grid_points": w.G, "n_samples": w.n_samples, "N": w.N, "M": w.M},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if w.precision == wl.PREC_F64 else "f32", "data": "synthetic",
+        "config": config_of(w, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle (unoptimised reference implementation)",
+                         "sample": sample, "single_core": {"value": v1, "seconds": dt1, "points": pts1}},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -164,13 +209,16 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2", choices=sorted(ALG_OPS))
+    ap.add_argument("--workload", default="cfg5", choices=sorted(ALG_OPS))
     ap.add_argument("--impl", default="zmc", choices=["zmc", "reference"])
     ap.add_argument("--schedule", type=int, default=0, help="0 auto, 1 thread, 2 warp, 3 cta")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the cfg1-cfg4 sub-records")
+    ap.add_argument("--no-pipe-rates", action="store_true")
     ap.add_argument("--adaptive", default="", help="n_first,n_max,target_stderr: also time zmc_scan_adaptive (N=1 only)")
-    ap.add_argument("--farm-devices", default="", help="e.g. 0,1,2,3: also time zmc_scan_farm over these devices (N=1 only)")
+    ap.add_argument("--farm-devices", default="", help="e.g. 0,1,2,3: also time zmc_scan_farm over these devices (N=1 only; "
+                    "default: all visible devices when there is more than one)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "zmc" else args.warmup
 
@@ -191,15 +239,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     zb.load()
-
-    w = build_workload(args.workload, world)
-    if w.name in USER_BODIES:
-        w.integrand_id = zb.zmc_register_integrand(w.name, USER_BODIES[w.name][1], w.N, w.M, len(w.consts))
-    G_scan = SCAN_POINTS.get(w.name, w.G) * (world if w.name in SCAN_POINTS else 1)
-    first, count = wl.shard_range(G_scan, rank, world)
     stream = torch.cuda.current_stream()
-    out_dtype = torch.float32 if w.out_f32 else torch.float64
-    elem = 4 if w.out_f32 else 8
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
     def barrier():
@@ -208,144 +248,193 @@ def main():
         torch.cuda.synchronize()
 
     def timed(fn, steps, warmup):
-        """K steps, each bracketed by CUDA events on the launching stream, L2 flushed in between."""
-        for _ in range(warmup):
-            fn()
+        """K steps, each bracketed by its own pair of CUDA events on the launching stream, L2 flushed in between (the
+        flush is outside the brackets).  The host does not synchronise between steps unless the step itself does
+        (timing=True): the queue stays full, so a bracket holds the step's device time, not the host's enqueue latency."""
+        t0 = time.perf_counter()
+        done = 0
+        while done < warmup or time.perf_counter() - t0 < 0.25:      # at least W steps AND a quarter second of work: a
+            fn()                                                      # 25-us step does not bring an idle GPU's clocks up
+            done += 1
+            if done % 64 == 0:
+                torch.cuda.synchronize()
         barrier()
-        total_ms, infos = 0.0, []
+        infos, events = [], []
         for _ in range(steps):
             flush.fill_(1)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
             infos.append(fn())
             b.record(stream)
-            b.synchronize()
-            total_ms += a.elapsed_time(b)
+            events.append((a, b))
         barrier()
+        total_ms = sum(a.elapsed_time(b) for a, b in events)
+
         if world > 1:
             t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             total_ms = float(t.item())
         return total_ms, infos
 
-    # ---- device-resident arm: `value` ---------------------------------------------------------------
-    # cfg5's 80 GB of results cannot stay in HBM next to nothing else on every pool GPU; like every
-    # config it is written to a device buffer here when that fits, else per-batch staging only (host arm).
-    device_fits = count * elem * 2 <= 100e9
-    if device_fits:
+    def measure(name, steps, warmup, want_e2e, e2e_steps):
+        """One workload: the device-resident arm (`value`), the HOST-output arm (`e2e`) and the roofline record."""
+        w = build_workload(name, world)
+        if w.name in USER_BODIES:
+            w.integrand_id = zb.zmc_register_integrand(w.name, USER_BODIES[w.name][1], w.N, w.M, len(w.consts))
+        cfg = config_of(w, world)
+        G_scan = cfg["scanned_points"]
+        first, count = wl.shard_range(G_scan, rank, world)
+        out_dtype = torch.float32 if w.out_f32 else torch.float64
+        elem = 4 if w.out_f32 else 8
+        common = dict(precision=w.precision, schedule=args.schedule, first_index=first, count=count, consts=w.consts)
+
+        # ---- device-resident arm: `value` (cfg5: its 80 GB of results fit a B200's 180 GB) ---------------------
+        if count * elem * 2 > 120e9:
+            raise SystemExit("workload does not fit the device-resident arm")
         d_mean = torch.empty(count, dtype=out_dtype, device="cuda")
         d_err = torch.empty(count, dtype=out_dtype, device="cuda")
-
-        def step_dev():
-            return zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, d_mean, d_err, stream,
-                                  precision=w.precision, schedule=args.schedule, batch_points=w.batch_points,
-                                  first_index=first, count=count, consts=w.consts, timing=True)
+        plan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, d_mean, d_err,
+                           batch_points=w.batch_points, **common)
+        # A step is the plain enqueue-only call a user makes.  For steps of a millisecond or more the library's own
+        # per-kernel events ride along in the timed steps (timing=True: negligible there); for tiny grids (cfg1: 25 us)
+        # that report's forced synchronisation would be most of the step, so the kernel time is taken in a second set of
+        # steps, timed the same way, right after.
+        plan(stream, timing=True)                   # first call: module load, list upload
+        probe = plan(stream, timing=True)
+        tiny = probe["kernel_ms"] < 1.0
         sampler = ClockSampler(local_rank)
         sampler.start()
-        total_ms, infos = timed(step_dev, args.steps, args.warmup)
+        total_ms, infos = timed((lambda: plan(stream)) if tiny else (lambda: plan(stream, timing=True)), steps, warmup)
+        if tiny:
+            _, infos = timed(lambda: plan(stream, timing=True), min(steps, 10), 1)
         clocks = sampler.stop()
         kernel_ms = float(np.mean([i["kernel_ms"] for i in infos]))
-        launches = int(sum(i["gpu_launches"] for i in infos))
+        launches = int(probe["gpu_launches"]) * steps + (int(sum(i["gpu_launches"] for i in infos)) if tiny else 0)
         sched = infos[-1]["schedule"]
-    else:
-        raise SystemExit("workload does not fit the device-resident arm")
+        ms_per_step = total_ms / steps
+        evals_all = G_scan * w.n_samples                   # all ranks together
+        evals_rank = count * w.n_samples
 
-    ms_per_step = total_ms / args.steps
-    evals_all = G_scan * w.n_samples                   # all ranks together
-    value = evals_all / (ms_per_step * 1e-3)
-    evals_rank = count * w.n_samples
+        adaptive = None
+        if args.adaptive and world == 1 and name == args.workload:
+            # NEXT-4: adaptive sample count; throughput counts the samples actually drawn (sum of out_n)
+            n_first, n_max, target = args.adaptive.split(",")
+            n_first, n_max, target = int(n_first), int(n_max), float(target)
+            a_n = torch.zeros(count, dtype=torch.int32, device="cuda")
 
-    # ---- end-to-end arm: HOST (pinned) outputs, D2H inside the timed region ------------------------------
-    e2e = None
-    if not args.no_e2e:
-        h_mean = torch.empty(count, dtype=out_dtype, pin_memory=True)
-        h_err = torch.empty(count, dtype=out_dtype, pin_memory=True)
-        bp = w.batch_points or max(1, min(count, 1 << 22))      # stream in batches so copies overlap compute
+            def step_adaptive():
+                return zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, n_first, n_max, target, w.seed, d_mean, d_err,
+                                            a_n, stream, precision=w.precision, first_index=first, count=count,
+                                            batch_points=w.batch_points, consts=w.consts, timing=True)
+            a_ms, _ = timed(step_adaptive, 3, 2)
+            drawn = int(a_n.to(torch.int64).sum().item())
+            adaptive = {"n_first": n_first, "n_max": n_max, "target_stderr": target, "ms_per_step": a_ms / 3,
+                        "samples_drawn": drawn, "value": drawn / (a_ms / 3 * 1e-3), "unit": UNIT,
+                        "mean_n": drawn / count, "frac_at_n_max": float((a_n == n_max).float().mean().item()),
+                        "fixed_n_max_evals": count * n_max}
+            del a_n
+        del plan, d_mean, d_err
+        torch.cuda.empty_cache()
 
-        def step_host():
-            return zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, stream,
-                                  precision=w.precision, schedule=args.schedule, batch_points=bp,
-                                  first_index=first, count=count, consts=w.consts, timing=True)
-        e_steps = max(2, min(args.steps, 5))
-        e_ms, e_infos = timed(step_host, e_steps, 1)
-        e2e = {"value": evals_all / (e_ms / e_steps * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": int(e_infos[-1]["h2d_bytes"]) * world,
-               "d2h_bytes_per_step": int(e_infos[-1]["d2h_bytes"]) * world,
-               "ms_per_step": e_ms / e_steps,
-               "kernel_ms": float(np.mean([i["kernel_ms"] for i in e_infos])),
-               "d2h_ms": float(np.mean([i["d2h_ms"] for i in e_infos])),
-               "exposed_d2h_ms": float(np.mean([i["exposed_d2h_ms"] for i in e_infos])),
-               "n_batches": int(e_infos[-1]["n_batches"]),
-               "d2h_gbs": float(np.mean([i["d2h_bytes"] / max(i["d2h_ms"], 1e-9) * 1e-6 for i in e_infos]))}
-        launches += int(sum(i["gpu_launches"] for i in e_infos))
+        # ---- end-to-end arm: HOST (pinned) outputs, list H2D forced and result D2H inside the timed region -------
+        e2e = farm = None
+        if want_e2e:
+            e_count = count if world == 1 else min(count, 1 << 31)       # bounded per rank when several ranks share one host
+            t0 = time.perf_counter()
+            h_mean = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
+            h_err = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
+            pin_s = time.perf_counter() - t0
+            bp = w.batch_points or max(1, min(e_count, 1 << 22))      # stream in batches so copies overlap compute
+            hplan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, batch_points=bp,
+                                flags=zb.ZMC_OPT_FRESH_LISTS, **dict(common, count=e_count))
+            e_ms, e_infos = timed(lambda: hplan(stream, timing=True), e2e_steps, 1)
+            e_evals_all = evals_all if e_count == count else e_count * w.n_samples * world
+            e2e = {"value": e_evals_all / (e_ms / e2e_steps * 1e-3), "unit": UNIT,
+                   "h2d_bytes_per_step": int(e_infos[-1]["h2d_bytes"]) * world,
+                   "d2h_bytes_per_step": int(e_infos[-1]["d2h_bytes"]) * world,
+                   "steps": e2e_steps, "ms_per_step": e_ms / e2e_steps,
+                   "scanned_points_per_rank": e_count,
+                   "kernel_ms": float(np.mean([i["kernel_ms"] for i in e_infos])),
+                   "d2h_ms": float(np.mean([i["d2h_ms"] for i in e_infos])),
+                   "exposed_d2h_ms": float(np.mean([i["exposed_d2h_ms"] for i in e_infos])),
+                   "n_batches": int(e_infos[-1]["n_batches"]), "host_out_pinned": int(e_infos[-1]["host_out_pinned"]),
+                   "pin_seconds_not_timed": pin_s,
+                   "d2h_gbs": float(np.mean([i["d2h_bytes"] / max(i["d2h_ms"], 1e-9) * 1e-6 for i in e_infos]))}
+            launches += int(sum(i["gpu_launches"] for i in e_infos))
+            # ---- NEXT-2: the single-node batch farm (host outputs, synchronous, host wall clock) -------------------
+            devs = [int(d) for d in args.farm_devices.split(",")] if args.farm_devices else \
+                (list(range(torch.cuda.device_count())) if torch.cuda.device_count() > 1 else [])
+            if devs and world == 1 and name == args.workload:
+                f_count = min(e_count, 1 << 31)
+                f_ms = []
+                for _ in range(3):
+                    tmf = zb.zmc_scan_farm(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean[:f_count], h_err[:f_count],
+                                           devs, precision=w.precision, schedule=args.schedule, first_index=first,
+                                           count=f_count, batch_points=min(w.batch_points or f_count, max(1, f_count // (4 * len(devs)))),
+                                           consts=w.consts)
+                    f_ms.append(tmf["wall_ms"])
+                farm = {"devices": devs, "value": f_count * w.n_samples / (min(f_ms[1:]) * 1e-3), "unit": UNIT,
+                        "wall_ms": min(f_ms[1:]), "scanned_points": f_count, "n_batches": tmf["n_batches"],
+                        "batches_done": tmf["batches_done"], "busy_ms": tmf["busy_ms"]}
+            del hplan, h_mean, h_err
 
-    # ---- NEXT-4: adaptive sample count; throughput counts the samples actually drawn (sum of out_n) -----------------
-    adaptive = None
-    if args.adaptive and world == 1:
-        n_first, n_max, target = args.adaptive.split(",")
-        n_first, n_max, target = int(n_first), int(n_max), float(target)
-        a_n = torch.zeros(count, dtype=torch.int32, device="cuda")
+        w_cyc, w_bound, w_res, w_add = w_min(w.name)
+        rate = evals_rank / (kernel_ms * 1e-3)
+        achieved = w_cyc * rate / 1e9
+        return {
+            "config": cfg, "w": w,
+            "value": evals_all / (ms_per_step * 1e-3), "points_per_s": G_scan / (ms_per_step * 1e-3),
+            "ms_per_step": ms_per_step, "kernel_ms_per_step": kernel_ms, "steps": steps, "warmup": warmup,
+            "schedule_used": {1: "thread", 2: "warp", 3: "cta"}[sched], "clocks": clocks, "e2e": e2e, "farm": farm,
+            "kernel_ms_from": "separate timed steps (library events force a sync)" if tiny else "the timed steps",
+            "adaptive": adaptive, "gpu_launches": launches,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
+                         "frac": achieved / PEAK_GLANE, "traffic": None,
+                         "lane_cycles_per_eval": w_cyc, "binding_resource": w_bound, "resources": w_res,
+                         "measured_lane_cycles_per_eval": PEAK_GLANE * 1e9 * (clocks["sm_mhz"] or SM_MAX_MHZ) / SM_MAX_MHZ / rate,
+                         "lane_cycles_per_eval_no_overlap": w_add, "frac_no_overlap": w_add * rate / 1e9 / PEAK_GLANE,
+                         "peak_source": "148 SMs x 4 SMSPs x 32 lanes x 1965 MHz dispatch; per-class costs: pipe_rates in this "
+                                        "line (zmc_measure_pipes), DESIGN.md section 6",
+                         "frac_at_measured_clock": (achieved / (PEAK_GLANE * clocks["sm_mhz"] / SM_MAX_MHZ)
+                                                    if clocks.get("sm_mhz") else None)},
+        }
 
-        def step_adaptive():
-            return zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, n_first, n_max, target, w.seed, d_mean, d_err,
-                                        a_n, stream, precision=w.precision, first_index=first, count=count,
-                                        batch_points=w.batch_points, consts=w.consts, timing=True)
-        a_ms, a_infos = timed(step_adaptive, 3, 2)
-        drawn = int(a_n.to(torch.int64).sum().item())
-        adaptive = {"n_first": n_first, "n_max": n_max, "target_stderr": target, "ms_per_step": a_ms / 3,
-                    "samples_drawn": drawn, "value": drawn / (a_ms / 3 * 1e-3), "unit": UNIT,
-                    "mean_n": drawn / count, "frac_at_n_max": float((a_n == n_max).float().mean().item()),
-                    "fixed_n_max_evals": count * n_max}
-
-    # ---- NEXT-2: the single-node batch farm over --farm-devices (host outputs, synchronous, host wall clock) -------
-    farm = None
-    if args.farm_devices and world == 1 and not args.no_e2e:
-        devs = [int(d) for d in args.farm_devices.split(",")]
-        f_ms = []
-        for _ in range(3):
-            tmf = zb.zmc_scan_farm(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, devs,
-                                   precision=w.precision, schedule=args.schedule, first_index=first, count=count,
-                                   batch_points=w.batch_points, consts=w.consts)
-            f_ms.append(tmf["wall_ms"])
-        farm = {"devices": devs, "value": evals_all / (min(f_ms[1:]) * 1e-3), "unit": UNIT, "wall_ms": min(f_ms[1:]),
-                "n_batches": tmf["n_batches"], "batches_done": tmf["batches_done"], "busy_ms": tmf["busy_ms"]}
+    main_rec = measure(args.workload, args.steps, args.warmup, not args.no_e2e, max(2, min(args.steps, 3)))
+    per_config = {}
+    if args.workload == "cfg5" and world == 1 and not args.no_per_config:
+        for name in PER_CONFIG:
+            r = measure(name, 10, 3, not args.no_e2e, 3)
+            r.pop("w")
+            per_config[name] = {k: r[k] for k in ("value", "points_per_s", "ms_per_step", "kernel_ms_per_step", "steps", "warmup",
+                                                  "schedule_used", "kernel_ms_from", "clocks", "roofline", "e2e", "gpu_launches")}
+            per_config[name]["grid_points"] = r["config"]["grid_points"]
+            per_config[name]["n_samples"] = r["config"]["n_samples"]
+    pipes = None
+    if not args.no_pipe_rates and rank == 0:
+        rep = zb.zmc_measure_pipes(stream)
+        pipes = {"sm_mhz": rep["sm_mhz"], "unit": "SMSP-cycles per group per warp: [measured, if independent pipes, if one shared pipe]",
+                 "rows": {r["name"]: [round(r["cycles"], 3), round(r["parallel"], 3), round(r["serial"], 3)] for r in rep["rows"]}}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    w_cyc, w_bound, w_res = w_min(w.name)
-    achieved = w_cyc * evals_rank / (kernel_ms * 1e-3) / 1e9
+    w = main_rec.pop("w")
+    launches = main_rec["gpu_launches"] + sum(p["gpu_launches"] for p in per_config.values())
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": (value / PUBLISHED_EVALS_PER_S[w.name] if w.name in PUBLISHED_EVALS_PER_S and world == 1 else None),
+        "metric": METRIC, "value": main_rec["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": main_rec["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": (main_rec["value"] / PUBLISHED_EVALS_PER_S[w.name] if w.name in PUBLISHED_EVALS_PER_S and world == 1 else None),
         "dtype": "f64" if w.precision == wl.PREC_F64 else "f32", "data": "synthetic",
-        "config": {"workload": w.name, "grid_points": w.G, "scanned_points": G_scan, "n_samples": w.n_samples,
-                   "N": w.N, "M": w.M, "evals_per_step": evals_all, "schedule": {1: "thread", 2: "warp", 3: "cta"}[sched],
-                   "accumulate": "f64", "l2_flush_between_steps": True, "seed": w.seed,
-                   "parallelism": f"index-range shards x{world}, no collective"},
-        "points_per_s": G_scan / (ms_per_step * 1e-3),
-        "kernel_ms_per_step": kernel_ms,
-        "clocks": clocks,
-        "e2e": e2e,
-        "farm": farm,
-        "adaptive": adaptive,
-        "gpu_launches": launches,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
-                     "frac": achieved / PEAK_GLANE, "traffic": None,
-                     "lane_cycles_per_eval": w_cyc, "binding_resource": w_bound, "resources": w_res,
-                     "measured_lane_cycles_per_eval": PEAK_GLANE * 1e9 * (clocks["sm_mhz"] or SM_MAX_MHZ) / SM_MAX_MHZ
-                     / (evals_rank / (kernel_ms * 1e-3)),
-                     "peak_source": "148 SMs x 4 SMSPs x 32 lanes x 1965 MHz dispatch; per-class costs measured by "
-                                    "paper_1910_01965_b200.pipe_rates (profiles/r01_pipe_rates.txt), DESIGN.md section 6",
-                     "frac_at_measured_clock": (achieved / (PEAK_GLANE * clocks["sm_mhz"] / SM_MAX_MHZ)
-                                                if clocks.get("sm_mhz") else None)},
+        "config": main_rec["config"],
+        "points_per_s": main_rec["points_per_s"], "kernel_ms_per_step": main_rec["kernel_ms_per_step"],
+        "schedule_used": main_rec["schedule_used"], "clocks": main_rec["clocks"], "e2e": main_rec["e2e"],
+        "farm": main_rec["farm"], "adaptive": main_rec["adaptive"], "gpu_launches": launches,
+        "roofline": main_rec["roofline"], "per_config": per_config or None, "pipe_rates": pipes,
     }
     if not args.no_cpu_baseline and world == 1:
-        v, cores, sample = cpu_oracle_rate(w)
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        out["cpu_baseline"] = cpu_baseline(w)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -10,12 +10,17 @@ LIB = os.path.join(HERE, "libzmc_oracle.so")
 
 
 def build(force: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
-        return LIB
+    import hashlib
     cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
            "-o", LIB + ".tmp", SRC, "-lm"]
+    stamp = hashlib.sha256(open(SRC, "rb").read() + " ".join(cmd).encode()).hexdigest()     # content, not file times
+    stamp_path = LIB + ".stamp"
+    if not force and os.path.exists(LIB) and os.path.exists(stamp_path) and open(stamp_path).read().strip() == stamp:
+        return LIB
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
+    with open(stamp_path, "w") as f:
+        f.write(stamp + "\n")
     return LIB
 
 

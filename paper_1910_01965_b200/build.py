@@ -46,12 +46,29 @@ def _newest(paths):
     return max(os.path.getmtime(p) for p in paths)
 
 
+def _source_stamp(srcs, deps) -> str:
+    """Hash of everything the library is built from.  File times are not trusted alone: a snapshot copied to another
+    machine (gpurun) arrives with shuffled mtimes, and a rebuild there costs half a minute of GPU time."""
+    import hashlib
+    h = hashlib.sha256(" ".join(FLAGS).encode())
+    for path in sorted(set(srcs + deps)):
+        h.update(os.path.basename(path).encode())
+        h.update(open(path, "rb").read())
+    return h.hexdigest()
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     deps = glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + \
         [os.path.join(HERE, "..", "include", "zmc.h")]
     os.makedirs(OBJ, exist_ok=True)
     deps.append(_write_rtc_headers())
+    stamp_path = LIB + ".stamp"
+    stamp = _source_stamp(srcs, deps)
+    if not force and os.path.exists(LIB) and os.path.exists(stamp_path) and open(stamp_path).read().strip() == stamp:
+        return LIB                                   # built from exactly these sources, whatever the file times say
+    if os.path.exists(stamp_path):
+        force = True                                 # sources changed since the stamped build: do not trust object times
     dep_time = _newest(deps)
     jobs = []
     objs = []
@@ -68,9 +85,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 if res.returncode:
                     raise RuntimeError("nvcc failed: " + " ".join(res.args))
     if jobs or not os.path.exists(LIB) or os.path.getmtime(LIB) < _newest(objs):
-        cmd = [NVCC, "-shared", "-o", LIB + ".tmp"] + objs + ["-ldl"]
+        cmd = [NVCC, "-Wno-deprecated-gpu-targets", "-shared", "-o", LIB + ".tmp"] + objs + ["-ldl"]
         subprocess.run(cmd, check=True)
         os.replace(LIB + ".tmp", LIB)
+    with open(stamp_path, "w") as f:
+        f.write(stamp + "\n")
     return LIB
 
 
