@@ -258,18 +258,35 @@ zmc_adapt_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_me
 
     uint32_t n_lo = 0, n_hi = p.n;                          // both multiples of S (validated on the host)
     double A, B, serr, inv_n;
+    // fp64: software-pipelined like the fixed-n kernel -- w always holds the lane's NEXT group, generated in the same
+    // basic block as the evaluation of the current one (the lane's groups l, l+32, ... run on across checkpoints, so the
+    // look-ahead carries over; the one group generated past the last checkpoint is discarded).  Same order of sums.
+    constexpr bool kPipelined = kN != 0 && std::is_same<R, double>::value;
+    uint32_t g_next = lane;
+    if constexpr (kPipelined) px.template blocks<GS::NB>(g_next * (uint32_t)GS::NB, p.rk, w);
     for (;;) {
-        for (uint32_t g = n_lo / S + lane; g < n_hi / S; g += 32u) {
-            const uint32_t j0 = g * (uint32_t)NB;
-            if constexpr (kN != 0) {
-                px.template blocks<GS::NB>(j0, p.rk, w);
-            } else {
+        if constexpr (kPipelined) {
+            for (; g_next < n_hi / S; g_next += 32u) {
+                R d[S];
 #pragma unroll
-                for (int b = 0; b < GS::NB; ++b)
-                    if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+                for (int s = 0; s < S; ++s) d[s] = fam.eval_shifted(&w[s * N], acc.K);
+                px.template blocks<GS::NB>((g_next + 32u) * (uint32_t)GS::NB, p.rk, w);
+#pragma unroll
+                for (int s = 0; s < S; ++s) acc.add_shifted(d[s]);
             }
+        } else {
+            for (uint32_t g = n_lo / S + lane; g < n_hi / S; g += 32u) {
+                const uint32_t j0 = g * (uint32_t)NB;
+                if constexpr (kN != 0) {
+                    px.template blocks<GS::NB>(j0, p.rk, w);
+                } else {
 #pragma unroll
-            for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
+                    for (int b = 0; b < GS::NB; ++b)
+                        if (b < NB) px.block(j0 + b, p.rk, *reinterpret_cast<uint32_t(*)[4]>(&w[4 * b]));
+                }
+#pragma unroll
+                for (int s = 0; s < S; ++s) acc.add_shifted(fam.eval_shifted(&w[s * N], acc.K));
+            }
         }
         A = acc.A; B = acc.B;                               // lane partials stay put; the tree works on copies
 #pragma unroll
