@@ -61,20 +61,29 @@ zmc_status farm_impl(int integrand_id, int N, const double* bounds, int M, const
     auto worker = [&](int slot) {
         cudaError_t ce = cudaSetDevice(devices[slot]);
         if (ce != cudaSuccess) { fail_cuda(ce); return; }
-        cudaStream_t stream = nullptr;
-        if ((ce = cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking)) != cudaSuccess) { fail_cuda(ce); return; }
-        cudaEvent_t inflight[2] = {nullptr, nullptr};          // at most two batches queued per device: the second one's
-        for (int i = 0; i < 2; ++i)                              // kernel overlaps the first one's D2H copy
-            if ((ce = cudaEventCreateWithFlags(&inflight[i], cudaEventDisableTiming)) != cudaSuccess) {
+        // At most two batches queued per device, on two alternating streams: every scan call ends by joining its result
+        // copies back into its stream, so on ONE stream the kernel of batch b+1 would wait for the copy of batch b
+        // (measured: 7 % on cfg 4); on the other stream it starts as soon as the SMs free up.
+        cudaStream_t streams[2] = {nullptr, nullptr};
+        cudaEvent_t inflight[2] = {nullptr, nullptr};
+        auto release = [&] {
+            for (int i = 0; i < 2; ++i) {
+                if (inflight[i]) cudaEventDestroy(inflight[i]);
+                if (streams[i]) cudaStreamDestroy(streams[i]);
+            }
+        };
+        for (int i = 0; i < 2; ++i)
+            if ((ce = cudaStreamCreateWithFlags(&streams[i], cudaStreamNonBlocking)) != cudaSuccess ||
+                (ce = cudaEventCreateWithFlags(&inflight[i], cudaEventDisableTiming)) != cudaSuccess) {
                 fail_cuda(ce);
-                if (inflight[0]) cudaEventDestroy(inflight[0]);
-                cudaStreamDestroy(stream);
+                release();
                 return;
             }
         bool used[2] = {false, false};
         const auto w0 = std::chrono::steady_clock::now();
         for (int64_t k = 0; failed == ZMC_OK; ++k) {
             const int e = (int)(k & 1);
+            cudaStream_t stream = streams[e];
             if (used[e] && (ce = cudaEventSynchronize(inflight[e])) != cudaSuccess) { fail_cuda(ce); break; }
             const int64_t b = next.fetch_add(1);
             if (b >= n_batches) break;
@@ -95,11 +104,10 @@ zmc_status farm_impl(int integrand_id, int N, const double* bounds, int M, const
             used[e] = true;
             ++done[slot];
         }
-        if ((ce = cudaStreamSynchronize(stream)) != cudaSuccess && failed == ZMC_OK) fail_cuda(ce);
+        for (int i = 0; i < 2; ++i)
+            if ((ce = cudaStreamSynchronize(streams[i])) != cudaSuccess && failed == ZMC_OK) fail_cuda(ce);
         busy_ms[slot] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - w0).count();
-        cudaEventDestroy(inflight[0]);
-        cudaEventDestroy(inflight[1]);
-        cudaStreamDestroy(stream);
+        release();
     };
 
     int prev = 0;
