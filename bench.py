@@ -59,6 +59,10 @@ USER_BODIES = {"cfg2_user": ("cfg2", "return zmc_sin(x[0] * y[0] + x[1] * y[1]);
                "cfg2_user_libdevice": ("cfg2", "return sin(x[0] * y[0] + x[1] * y[1]);")}
 PUBLISHED_EVALS_PER_S = {"eq4": 1e6 * 1e5 / 18.19497}
 PER_CONFIG = ["cfg1", "cfg2", "cfg3", "cfg4"]
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of the scan kernel, per launch, from the one
+# `ncu --set full` capture of each kernel (profiles/r02_kernel.md).  cfg5: per 2^28-point batch launch (algorithmic:
+# 2^28 x 8 B = 2.147e9 written); cfg4: 1e8 x 16 B = 1.6e9; cfg2: its 16 MB of results never leave L2 during the kernel.
+NCU_TRAFFIC_BYTES = {"cfg5": 28.094464e6 + 2.096151e9, "cfg4": 37.298176e6 + 1.556428e9, "cfg2": 40.96e3 + 0.0}
 
 
 def w_min(name):
@@ -389,7 +393,7 @@ def main():
             "kernel_ms_from": "separate timed steps (library events force a sync)" if tiny else "the timed steps",
             "adaptive": adaptive, "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
-                         "frac": achieved / PEAK_GLANE, "traffic": None,
+                         "frac": achieved / PEAK_GLANE, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
                          "lane_cycles_per_eval": w_cyc, "binding_resource": w_bound, "resources": w_res,
                          "measured_lane_cycles_per_eval": PEAK_GLANE * 1e9 * (clocks["sm_mhz"] or SM_MAX_MHZ) / SM_MAX_MHZ / rate,
                          "lane_cycles_per_eval_no_overlap": w_add, "frac_no_overlap": w_add * rate / 1e9 / PEAK_GLANE,
