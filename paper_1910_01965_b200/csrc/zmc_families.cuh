@@ -128,7 +128,7 @@ template <typename R, bool FAST> struct FamC4 {
         }
         return Fn<R, FAST>::exp2_neg(acc);
     }
-    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return Real<R>::sub(eval(w), K); }
 };
 
 // c5: exp(-x1 |y|^2) cos(x2 y0 + x3 y1 + x4 y2) (1 + x5 y0 y1 y2)      (configs[4])
@@ -172,7 +172,7 @@ template <typename R> struct FamConstOne {
     static constexpr int kN = 0;
     __device__ __forceinline__ void setup(const R*, const ScanParams&) {}
     __device__ __forceinline__ R eval(const uint32_t*) const { return (R)1; }
-    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return Real<R>::sub(eval(w), K); }
 };
 
 template <typename R> struct FamParamEcho {
@@ -187,7 +187,7 @@ template <typename R> struct FamParamEcho {
             if (l == i) v = x[l];
     }
     __device__ __forceinline__ R eval(const uint32_t*) const { return v; }
-    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return Real<R>::sub(eval(w), K); }
 };
 
 template <typename R> struct FamLinY {
@@ -203,7 +203,7 @@ template <typename R> struct FamLinY {
     __device__ __forceinline__ R eval(const uint32_t* w) const {
         return Real<R>::fma(uniform<R>(w[k]), width, a);
     }
-    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return Real<R>::sub(eval(w), K); }
 };
 
 template <typename R> struct FamPoly {
@@ -217,7 +217,7 @@ template <typename R> struct FamPoly {
             prod *= Real<R>::fma(uniform<R>(w[k]), (R)pp->width[k], (R)pp->a[k]);
         return prod;
     }
-    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return Real<R>::sub(eval(w), K); }
 };
 
 }  // namespace zmc

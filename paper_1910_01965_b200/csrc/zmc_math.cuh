@@ -108,6 +108,9 @@ template <> struct Real<float> {
     static __device__ __forceinline__ double u_scale() { return 1.0; }
     static __device__ __forceinline__ double u_offset() { return 0x1.fffffep-1; }          // 1 - 2^-24
     static __device__ __forceinline__ float fma(float a, float b, float c) { return fmaf(a, b, c); }
+    // a - b that the compiler may NOT contract with a multiply feeding a (g - K must round the same way in every kernel
+    // a family is compiled into: the adaptive scan is bit-identical to the fixed-n scan)
+    static __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
 };
 
 template <> struct Real<double> {
@@ -124,6 +127,7 @@ template <> struct Real<double> {
     static __device__ __forceinline__ double u_offset() { return 0x1.ffffffffp-1; }        // 1 - 2^-33
 #endif
     static __device__ __forceinline__ double fma(double a, double b, double c) { return ::fma(a, b, c); }
+    static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
 };
 
 // exact lattice uniform u in (0,1) (diagnostic families; the hot families fold scale and offset)
@@ -203,7 +207,7 @@ template <> struct Fn<float, false> {
     static constexpr double kQuarter = 1.5707963267948966;
     static __device__ __forceinline__ double wrap(double c) { return c - 6.283185307179586 * rint(c * 0.15915494309189533577); }
     static __device__ __forceinline__ float sin_phase(float a) { return sinf(a); }
-    static __device__ __forceinline__ float sin_phase_minus(float a, float K) { return sinf(a) - K; }
+    static __device__ __forceinline__ float sin_phase_minus(float a, float K) { return __fsub_rn(sinf(a), K); }
     static __device__ __forceinline__ float exp2_neg(float e) { return exp2f(-e); }
 };
 

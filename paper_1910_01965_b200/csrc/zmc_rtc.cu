@@ -125,7 +125,7 @@ template <typename R> struct FamUser {
         for (int k = 0; k < ZMC_USER_N; ++k) y[k] = Real<R>::fma(uniform<R>(w[k]), wd[k], a[k]);
         return g(y, xs, cs);
     }
-    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return eval(w) - K; }
+    __device__ __forceinline__ R eval_shifted(const uint32_t* w, R K) const { return Real<R>::sub(eval(w), K); }      // never contracted into g's last multiply
 };
 }  // namespace zmc
 )SRC";
