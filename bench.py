@@ -345,8 +345,16 @@ def main():
         if want_e2e:
             e_count = count if world == 1 else min(count, 1 << 31)       # bounded per rank when several ranks share one host
             t0 = time.perf_counter()
-            h_mean = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
-            h_err = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
+            while True:          # 80 GB of page-locked memory for cfg5: if this host cannot pin that much, scan (and say) less
+                try:
+                    h_mean = h_err = None
+                    h_mean = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
+                    h_err = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
+                    break
+                except RuntimeError:
+                    if e_count <= (1 << 28):
+                        raise
+                    e_count = max(1 << 28, e_count // 2)
             pin_s = time.perf_counter() - t0
             bp = w.batch_points or max(1, min(e_count, 1 << 22))      # stream in batches so copies overlap compute
             hplan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, batch_points=bp,
