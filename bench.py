@@ -291,6 +291,7 @@ def main():
         out_dtype = torch.float32 if w.out_f32 else torch.float64
         elem = 4 if w.out_f32 else 8
         common = dict(precision=w.precision, schedule=args.schedule, first_index=first, count=count, consts=w.consts)
+        shard_flags = zb.ZMC_OPT_EXPLICIT_COUNT if world > 1 else 0        # a rank's shard may be empty: count is meant literally
 
         # ---- device-resident arm: `value` (cfg5: its 80 GB of results fit a B200's 180 GB) ---------------------
         if count * elem * 2 > 120e9:
@@ -298,7 +299,7 @@ def main():
         d_mean = torch.empty(count, dtype=out_dtype, device="cuda")
         d_err = torch.empty(count, dtype=out_dtype, device="cuda")
         plan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, d_mean, d_err,
-                           batch_points=w.batch_points, **common)
+                           batch_points=w.batch_points, flags=shard_flags, **common)
         # A step is the plain enqueue-only call a user makes.  For steps of a millisecond or more the library's own
         # per-kernel events ride along in the timed steps (timing=True: negligible there); for tiny grids (cfg1: 25 us)
         # that report's forced synchronisation would be most of the step, so the kernel time is taken in a second set of
@@ -358,7 +359,7 @@ def main():
             pin_s = time.perf_counter() - t0
             bp = w.batch_points or max(1, min(e_count, 1 << 22))      # stream in batches so copies overlap compute
             hplan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, batch_points=bp,
-                                flags=zb.ZMC_OPT_FRESH_LISTS, **dict(common, count=e_count))
+                                flags=zb.ZMC_OPT_FRESH_LISTS | shard_flags, **dict(common, count=e_count))
             e_ms, e_infos = timed(lambda: hplan(stream, timing=True), e2e_steps, 1)
             e_evals_all = evals_all if e_count == count else e_count * w.n_samples * world
             e2e = {"value": e_evals_all / (e_ms / e2e_steps * 1e-3), "unit": UNIT,

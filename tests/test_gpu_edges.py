@@ -123,3 +123,38 @@ def test_back_to_back_host_output_scans_on_two_streams_and_after_shutdown():
     zb.zmc_shutdown()
     m2, e2 = run_gpu(ws[0], schedule=1)
     assert np.array_equal(m2, refs[0][0]) and np.array_equal(e2, refs[0][1])
+
+
+def test_measure_pipes_reports_the_dispatch_costs_the_roofline_uses():
+    """zmc_measure_pipes (include/zmc.h): the rows bench.py prints as `pipe_rates`.  Sanity bands only -- the numbers are
+    measurements -- around what DESIGN.md section 6 builds the ALU roofline from: integer 2 cycles per warp-instruction,
+    FP32 1, FP64 2, XU 8, and a `serial >= parallel` pair of bounds on every mixed row."""
+    from paper_1910_01965_b200 import binding as zb
+    rep = zb.zmc_measure_pipes()
+    rows = {r["name"]: r for r in rep["rows"]}
+    assert rep["sm_count"] >= 1 and 500.0 < rep["sm_mhz"] < 3000.0 and len(rows) >= 30
+    for name, lo, hi in [("LOP3", 1.8, 2.6), ("SHF", 1.8, 2.6), ("IMAD.WIDE+LOP3", 3.6, 5.0), ("FFMA", 0.9, 1.5),
+                         ("DFMA", 1.8, 2.6), ("DADD", 1.8, 2.6), ("MUFU.EX2", 7.0, 9.5), ("F2F.F64.F32", 7.0, 9.5)]:
+        assert lo < rows[name]["cycles"] < hi, (name, rows[name])
+    for r in rep["rows"]:
+        assert r["serial"] >= r["parallel"] > 0 and 0.8 * r["parallel"] < r["cycles"] < 1.25 * r["serial"], r
+    both = rows["cfg2 block: both, same warp (ptxas order)"]
+    assert both["parallel"] < both["cycles"] < both["serial"]
+
+
+def test_scan_plan_is_the_same_call_and_an_explicitly_empty_shard_is_a_no_op():
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(3, scale=[5, 4, 6], n_samples=300)
+    m, e, _ = zb.scan_workload(w)
+    pm, pe = torch.full_like(m, -3.0), torch.full_like(e, -3.0)
+    plan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, pm, pe, precision=w.precision, consts=w.consts)
+    tm = plan(None, timing=True)
+    torch.cuda.synchronize()
+    assert torch.equal(pm, m) and torch.equal(pe, e) and tm["gpu_launches"] == 1
+    pm.fill_(-3.0)
+    empty = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, pm, pe, precision=w.precision, consts=w.consts,
+                        first_index=7, count=0, flags=zb.ZMC_OPT_EXPLICIT_COUNT)
+    tm = empty(None, timing=True)
+    torch.cuda.synchronize()
+    assert tm["gpu_launches"] == 0 and bool((pm == -3.0).all())
