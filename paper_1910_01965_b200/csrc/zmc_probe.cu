@@ -23,7 +23,8 @@ namespace {
 
 #define ZMC_PROBE_M0 0xD2511F53u
 
-enum Op { LOP3, SHF, WL /* IMAD.WIDE.U32 + the LOP3 that eats both halves: a Philox half-round */, FFMA, DFMA, DADD, MUFU, F2F, NONE };
+enum Op { LOP3, SHF, WL /* IMAD.WIDE.U32 + the LOP3 that eats both halves: a Philox half-round */, FFMA, DFMA, DADD, MUFU, F2F,
+          IMADLO /* 32-bit product, low half only */, IMADHI, NONE };
 
 struct Regs {
     uint32_t c0[8], c1[8], e[8];
@@ -58,6 +59,8 @@ template <int OP> __device__ __forceinline__ void emit(Regs& r, int i, uint32_t 
         asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(r.c0[i]), "n"(ZMC_PROBE_M0));
         asm volatile("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r.c0[i]) : "r"((uint32_t)(p >> 32)), "r"((uint32_t)p), "r"(k));
     }
+    if (OP == IMADLO) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r.c1[i]) : "n"(ZMC_PROBE_M0), "r"(r.c1[(i + 1) & 7]));
+    if (OP == IMADHI) asm volatile("mad.hi.u32 %0, %0, %1, %2;" : "+r"(r.c1[i]) : "n"(ZMC_PROBE_M0), "r"(r.c1[(i + 1) & 7]));
     if (OP == FFMA) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(r.f[i]) : "f"(fk), "f"(fc));
     if (OP == DFMA) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(r.d[i]) : "d"(dk), "d"(dc));
     if (OP == DADD) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(r.d[i]) : "d"(dk));
@@ -123,6 +126,96 @@ __global__ void __launch_bounds__(256) probe_block(uint32_t* out, int iters, uin
     out[blockIdx.x * blockDim.x + threadIdx.x] = fold(r);
 }
 
+
+// ------------------------------------------------------------------------------------------------------------------
+// What a Philox4x32-10 block costs and WHY.  Three blocks in lock-step per thread, per-thread
+// rounds 3-10 (16 multiplies + 18 three-input XORs per block, the library's own formulation; the block index is
+// warp-uniform as in the THREAD schedule), in four variants:
+//   kWide   the real thing: IMAD.WIDE.U32 gives both halves of each 32x32 product
+//   kLowOnly  the same dataflow with the LOW halves only (IMAD.LO) -- NOT Philox, a control: shows that a 32-bit product
+//             overlaps with the XORs and that it is the HIGH half of the product that costs
+//   kHiF64  the real thing again, high halves from the FP64 pipe: with D = 2^52 + c held as a double,
+//             fma.rz(D, M 2^-32, 2^52 - M 2^20) = 2^52 + floor(c M / 2^32) exactly, low halves by IMAD.LO (bit-identical output)
+// plus EXTRA independent instructions of one class per block next to the real thing: the slope says what an instruction
+// of that class costs inside the Philox stream (FFMA ~1, LOP3 ~2: they add, nothing hides).
+enum PhiloxVariant { kWide, kLowOnly, kHiF64 };
+#define ZMC_PROBE_M1 0xCD9E8D57u
+struct ProbeKeys { uint32_t rk[20]; };
+
+template <int VARIANT, int NB>
+__device__ __forceinline__ void probe_philox_blocks(uint32_t e0, uint32_t e2, uint32_t c3i, uint32_t j0, const ProbeKeys& K, uint32_t* out) {
+    if (VARIANT == kHiF64) {
+        const double M0s = (double)ZMC_PROBE_M0 * 0x1p-32, M1s = (double)ZMC_PROBE_M1 * 0x1p-32;
+        const double C0 = 0x1p52 - (double)ZMC_PROBE_M0 * 0x1p20, C1 = 0x1p52 - (double)ZMC_PROBE_M1 * 0x1p20;
+        const unsigned long long kMagic = 0x4330000000000000ull;
+        unsigned long long D0[NB], D2[NB];
+        uint32_t c1[NB], c3[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const uint64_t p0 = (uint64_t)ZMC_PROBE_M0 * (j0 + (uint32_t)b);
+            const uint64_t p1 = (uint64_t)ZMC_PROBE_M1 * ((uint32_t)(p0 >> 32) ^ K.rk[1]);
+            D0[b] = kMagic | ((uint32_t)(p1 >> 32) ^ e0); c1[b] = (uint32_t)p1; D2[b] = kMagic | (e2 ^ (uint32_t)p0); c3[b] = c3i;
+        }
+#pragma unroll
+        for (int r = 2; r < 10; ++r)
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                double h0, h2;
+                asm("fma.rz.f64 %0, %1, %2, %3;" : "=d"(h0) : "d"(__longlong_as_double((long long)D0[b])), "d"(M0s), "d"(C0));
+                asm("fma.rz.f64 %0, %1, %2, %3;" : "=d"(h2) : "d"(__longlong_as_double((long long)D2[b])), "d"(M1s), "d"(C1));
+                const uint32_t lo0 = (uint32_t)D0[b] * ZMC_PROBE_M0, lo1 = (uint32_t)D2[b] * ZMC_PROBE_M1;
+                D0[b] = (unsigned long long)__double_as_longlong(h2) ^ (unsigned long long)(c1[b] ^ K.rk[2 * r]);
+                D2[b] = (unsigned long long)__double_as_longlong(h0) ^ (unsigned long long)(c3[b] ^ K.rk[2 * r + 1]);
+                c1[b] = lo1; c3[b] = lo0;
+            }
+#pragma unroll
+        for (int b = 0; b < NB; ++b) { out[4 * b] = (uint32_t)D0[b]; out[4 * b + 1] = c1[b]; out[4 * b + 2] = (uint32_t)D2[b]; out[4 * b + 3] = c3[b]; }
+    } else {
+        uint32_t c0[NB], c1[NB], c2[NB], c3[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const uint64_t p0 = (uint64_t)ZMC_PROBE_M0 * (j0 + (uint32_t)b);
+            const uint64_t p1 = (uint64_t)ZMC_PROBE_M1 * ((uint32_t)(p0 >> 32) ^ K.rk[1]);
+            c0[b] = (uint32_t)(p1 >> 32) ^ e0; c1[b] = (uint32_t)p1; c2[b] = e2 ^ (uint32_t)p0; c3[b] = c3i;
+        }
+#pragma unroll
+        for (int r = 2; r < 10; ++r)
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                if (VARIANT == kWide) {
+                    const uint64_t p0 = (uint64_t)ZMC_PROBE_M0 * c0[b], p1 = (uint64_t)ZMC_PROBE_M1 * c2[b];
+                    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1[b] ^ K.rk[2 * r], n2 = (uint32_t)(p0 >> 32) ^ c3[b] ^ K.rk[2 * r + 1];
+                    c1[b] = (uint32_t)p1; c3[b] = (uint32_t)p0; c0[b] = n0; c2[b] = n2;
+                } else {
+                    const uint32_t q0 = ZMC_PROBE_M0 * c0[b], q1 = ZMC_PROBE_M1 * c2[b];
+                    const uint32_t n0 = q1 ^ c1[b] ^ K.rk[2 * r], n2 = q0 ^ c3[b] ^ K.rk[2 * r + 1];
+                    c1[b] = q1; c3[b] = q0; c0[b] = n0; c2[b] = n2;
+                }
+            }
+#pragma unroll
+        for (int b = 0; b < NB; ++b) { out[4 * b] = c0[b]; out[4 * b + 1] = c1[b]; out[4 * b + 2] = c2[b]; out[4 * b + 3] = c3[b]; }
+    }
+}
+
+template <int VARIANT, int EXTRA_OP, int EXTRA>
+__global__ void __launch_bounds__(256, 4) probe_philox(uint32_t* out, int iters, uint32_t k, float fk, float fc, double dk, double dc,
+                                                        const __grid_constant__ ProbeKeys K) {
+    constexpr int NB = 3;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t e0 = tid * 2654435761u, e2 = tid * 40503u + 7u, c3i = tid ^ 0x55u;
+    Regs r;
+    init(r, tid, k);
+    uint32_t acc = 0, w[4 * NB];
+    for (int it = 0; it < iters; ++it) {
+        probe_philox_blocks<VARIANT, NB>(e0, e2, c3i, (uint32_t)(it * NB), K, w);
+        burst<EXTRA_OP, EXTRA * NB>(r, 0, k, fk, fc, dk, dc);
+#pragma unroll
+        for (int i = 0; i < 4 * NB; ++i) acc += w[i];          // consumer: one three-input add per two words (a sum: XOR would cancel
+                                                                // the last round of the low-halves-only control)
+    }
+    out[tid] = acc ^ fold(r);
+}
+
 __global__ void probe_clock(long long* out) {
     const long long c0 = clock64();
     unsigned long long g0, g1;
@@ -132,7 +225,7 @@ __global__ void probe_clock(long long* out) {
     out[1] = (long long)(g1 - g0);
 }
 
-const char* kName[] = {"LOP3", "SHF", "IMAD.WIDE+LOP3", "FFMA", "DFMA", "DADD", "MUFU.EX2", "F2F.F64.F32", ""};
+const char* kName[] = {"LOP3", "SHF", "IMAD.WIDE+LOP3", "FFMA", "DFMA", "DADD", "MUFU.EX2", "F2F.F64.F32", "IMAD.LO", "IMAD.HI", ""};
 
 struct Probe {
     cudaStream_t stream;
@@ -214,7 +307,10 @@ extern "C" zmc_status zmc_measure_pipes(zmc_pipe_report* report, void* stream_v)
 
     const double lop = p.alone<LOP3>(), shf = p.alone<SHF>(), wl = p.alone<WL>(), ffma = p.alone<FFMA>();
     const double dfma = p.alone<DFMA>(), dadd = p.alone<DADD>(), mufu = p.alone<MUFU>(), f2f = p.alone<F2F>();
+    const double imadlo = p.alone<IMADLO>();
+    p.alone<IMADHI>();
     (void)shf; (void)dadd;
+    p.pair<IMADLO, 1, LOP3, 1>(imadlo, lop);
     p.pair<LOP3, 1, DFMA, 1>(lop, dfma);
     p.pair<LOP3, 1, DADD, 1>(lop, dadd);
     p.pair<WL, 1, DFMA, 2>(wl, dfma);
@@ -238,6 +334,21 @@ extern "C" zmc_status zmc_measure_pipes(zmc_pipe_report* report, void* stream_v)
         p.add("cfg2 block: FP64 part alone (32 DFMA)", cd, cd, cd);
         p.add("cfg2 block: both, same warp (ptxas order)", cm, par, ci + cd);
         p.add("cfg2 block: integer warps | FP64 warps", cs, par, ci + cd);
+    }
+
+    {   // one Philox block inside the stream of the THREAD schedule (three blocks in lock-step, 8 warps per SMSP)
+        ProbeKeys K;
+        for (int r = 0; r < 10; ++r) { K.rk[2 * r] = 0xDEADBEEFu + r * 0x9E3779B9u; K.rk[2 * r + 1] = 0x12345678u + r * 0xBB67AE85u; }
+        const int it = 1500;
+        auto blk = [&](double ms) { return p.cycles(ms, 3.0 * it, 8.0); };
+        const double alu = 18 * lop, all = 34 * lop;       // XORs alone | every integer instruction at the ALU rate
+        const double base = blk(p.time_ms(probe_philox<kWide, NONE, 0>, p.out, it, 12345u, 0.999f, 1e-3f, 0.999, 1e-3, K));
+        p.add("Philox block: 16 IMAD.WIDE + 18 LOP3 per thread + uniform rounds 1-2", base, alu, all);
+        p.add("  + 8 independent FFMA per block", blk(p.time_ms(probe_philox<kWide, FFMA, 8>, p.out, it, 12345u, 0.999f, 1e-3f, 0.999, 1e-3, K)), base, base + 8 * ffma);
+        p.add("  + 8 independent DFMA per block", blk(p.time_ms(probe_philox<kWide, DFMA, 8>, p.out, it, 12345u, 0.999f, 1e-3f, 0.999, 1e-3, K)), base, base + 8 * dfma);
+        p.add("  + 8 independent LOP3 per block", blk(p.time_ms(probe_philox<kWide, LOP3, 8>, p.out, it, 12345u, 0.999f, 1e-3f, 0.999, 1e-3, K)), base, base + 8 * lop);
+        p.add("  control: low halves only (16 IMAD.LO + 18 LOP3; NOT Philox)", blk(p.time_ms(probe_philox<kLowOnly, NONE, 0>, p.out, it, 12345u, 0.999f, 1e-3f, 0.999, 1e-3, K)), alu, 16 * imadlo + alu);
+        p.add("  high halves by DFMA.RZ (FP64 pipe) + IMAD.LO: same output", blk(p.time_ms(probe_philox<kHiF64, NONE, 0>, p.out, it, 12345u, 0.999f, 1e-3f, 0.999, 1e-3, K)), alu, 16 * imadlo + alu + 16 * dfma);
     }
     cudaEventDestroy(p.a);
     cudaEventDestroy(p.b);
