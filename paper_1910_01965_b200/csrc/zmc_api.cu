@@ -370,8 +370,11 @@ zmc_status zmc_validate(int integrand_id, int N, const double* bounds, int M, co
 // H6 schedule choice.  R = threads the device keeps resident: the fp64 kernels are launch-bounded to 3 CTAs of 256
 // per SM, the fp32-evaluate ones to 4 (zmc_kernel.cuh); the SM count is the current device's (148 on a B200, also the
 // fallback when no device is visible).  THREAD needs >= 8 rounds of R (measured on cfg 2, 8.8 rounds: 2.8 % faster
-// than WARP because rounds 1-2 of Philox run on the uniform datapath); WARP the same in warps; else CTA.  A point with
-// few sample groups cannot feed 32 / 256 lanes, so small n falls back to fewer lanes.
+// than WARP because rounds 1-2 of Philox run on the uniform datapath); WARP needs 2 rounds of R/32 resident warps
+// (measured on B200 for the cfg 1-3 families with 2000-16000 points x 5000-50000 samples: below that the finer
+// granularity of one CTA per point wins by up to 20 %, above it WARP by 5-15 % -- one shuffle tree instead of a tree,
+// a barrier and a second tree per point); else CTA.  A point with few sample groups cannot feed 32 / 256 lanes, so
+// small n falls back to fewer lanes.
 static int cached_sm_count() {
     static int sms = [] {
         int dev = 0, n = 0;
@@ -389,7 +392,7 @@ int zmc_pick_schedule_ex(uint64_t count, uint64_t n_samples, int N, int precisio
     const int g4 = (N % 4 == 0) ? 4 : (N % 2 == 0) ? 2 : 1;
     const uint64_t groups = n_samples / (uint64_t)(4 / g4) + 1;
     if (count >= 8 * resident || groups < 4 * 32) return ZMC_SCHED_THREAD;
-    if (count >= 8 * (resident / 32) || groups < 4 * 256) return ZMC_SCHED_WARP;
+    if (count >= 2 * (resident / 32) || groups < 4 * 256) return ZMC_SCHED_WARP;
     return ZMC_SCHED_CTA;
 }
 

@@ -102,6 +102,10 @@ def test_schedule_choice_follows_design_table():
     assert zb.zmc_pick_schedule(10 ** 5, 10 ** 4, 2) == zb.ZMC_SCHED_WARP
     assert zb.zmc_pick_schedule(10 ** 6, 10 ** 4, 2, zb.ZMC_PREC_F64) == zb.ZMC_SCHED_THREAD
     assert zb.zmc_pick_schedule(10 ** 6, 10 ** 4, 2, zb.ZMC_PREC_F32E) == zb.ZMC_SCHED_WARP
+    # WARP from two rounds of resident warps (148 SMs x 24 fp64 / 32 fp32-evaluate warps), one CTA per point below that
+    assert zb.zmc_pick_schedule(7000, 10 ** 4, 2) == zb.ZMC_SCHED_CTA and zb.zmc_pick_schedule(7200, 10 ** 4, 2) == zb.ZMC_SCHED_WARP
+    assert zb.zmc_pick_schedule(9400, 10 ** 4, 4, zb.ZMC_PREC_F32E) == zb.ZMC_SCHED_CTA
+    assert zb.zmc_pick_schedule(9500, 10 ** 4, 4, zb.ZMC_PREC_F32E) == zb.ZMC_SCHED_WARP
 
 
 def test_explicit_count_makes_an_empty_range_expressible():
