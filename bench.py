@@ -354,10 +354,10 @@ def main():
             while True:          # 80 GB of page-locked memory for cfg5: if this host cannot pin that much, scan (and say) less
                 try:
                     h_mean = h_err = None
-                    h_mean = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
-                    h_err = torch.empty(e_count, dtype=out_dtype, pin_memory=True)
+                    h_mean = zb.pinned_empty(e_count, out_dtype)
+                    h_err = zb.pinned_empty(e_count, out_dtype)
                     break
-                except RuntimeError:
+                except (RuntimeError, MemoryError, OSError):
                     if e_count <= (1 << 28):
                         raise
                     e_count = max(1 << 28, e_count // 2)

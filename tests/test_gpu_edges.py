@@ -168,3 +168,27 @@ def test_scan_plan_is_the_same_call_and_an_explicitly_empty_shard_is_a_no_op():
     tm = empty(None, timing=True)
     torch.cuda.synchronize()
     assert tm["gpu_launches"] == 0 and bool((pm == -3.0).all())
+
+
+def test_pinned_empty_is_page_locked_host_memory_the_library_streams_into():
+    """binding.pinned_empty (memory plumbing for HOST outputs): parallel first touch + cudaHostRegister.  The library must
+    see the buffer as pinned (zmc_timing.host_out_pinned == 1) and the scan through it must equal the device-output scan."""
+    import gc
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(5, scale=[8] * 5, n_samples=64)
+    count = 1 << 25                                     # 128 MiB per fp32 array: above the helper's small-size fallback
+    big = zb.pinned_empty(count, torch.float32, fill=float("nan"))
+    err = zb.pinned_empty(count, torch.float32, fill=float("nan"))
+    assert big.is_pinned() and err.is_pinned() and bool(torch.isnan(big[::4099]).all())
+    m, e, tm = zb.scan_workload(w, out_mean=big[:w.G], out_stderr=err[:w.G], host_out=True, batch_points=10_000, timing=True)
+    torch.cuda.synchronize()
+    assert tm["host_out_pinned"] == 1 and tm["n_batches"] == 4
+    dm, de, _ = zb.scan_workload(w, host_out=False)
+    torch.cuda.synchronize()
+    assert torch.equal(m, dm.cpu()) and torch.equal(e, de.cpu())
+    assert bool(torch.isnan(big[w.G:w.G + 1000]).all())           # nothing written past the range
+    small = zb.pinned_empty(1000, torch.float64)                  # small sizes: torch's own pinned allocator
+    assert small.is_pinned() and small.numel() == 1000
+    del big, err, m, e
+    gc.collect()                                                   # the registration is undone with the tensor
