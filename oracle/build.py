@@ -5,8 +5,10 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "zmc_oracle.c")
-LIB = os.path.join(HERE, "libzmc_oracle.so")
+# ZMC_ORACLE_SRC / ZMC_ORACLE_LIB: build and load another copy of the source instead -- used only by
+# tests/test_oracle_mutations.py, which checks that a deliberately broken oracle turns the pin tests red.
+SRC = os.environ.get("ZMC_ORACLE_SRC") or os.path.join(HERE, "zmc_oracle.c")
+LIB = os.environ.get("ZMC_ORACLE_LIB") or os.path.join(HERE, "libzmc_oracle.so")
 
 
 def build(force: bool = False) -> str:
