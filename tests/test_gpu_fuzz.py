@@ -46,8 +46,18 @@ def test_random_configuration_matches_oracle(case):
     w, opts = draw(case)
     rc, mean_o, err_o = orc.scan_workload(w, opts["first_index"], opts["count"], n_threads=NT)
     assert rc == 0, (w, opts)
-    m, e, _ = zb.scan_workload(w, **opts)
+    # outputs sit inside guard zones of NaN (compute-sanitizer is closed on this GPU pool): a write outside
+    # [0, count) of either array -- on the device or, with host outputs, by the result copies -- shows up here
+    pad, count = 96, opts["count"]
+    dt = torch.float32 if w.out_f32 else torch.float64
+    mk = (lambda: torch.full((count + 2 * pad,), float("nan"), dtype=dt).pin_memory()) if opts["host_out"] else \
+         (lambda: torch.full((count + 2 * pad,), float("nan"), dtype=dt, device="cuda"))
+    gm, ge = mk(), mk()
+    m, e, _ = zb.scan_workload(w, out_mean=gm[pad:pad + count], out_stderr=ge[pad:pad + count], **opts)
     torch.cuda.synchronize()
+    for g in (gm, ge):
+        assert bool(torch.isnan(g[:pad]).all()) and bool(torch.isnan(g[pad + count:]).all()), "write outside the output range"
+        assert not bool(torch.isnan(g[pad:pad + count]).any()), "an element of the range was not written"
     b = np.asarray(w.bounds).reshape(-1, 2)
     volume = float(np.prod(b[:, 1] - b[:, 0]))
     assert_parity(w, m.cpu().numpy(), e.cpu().numpy(), mean_o, err_o, abs_scale=max(1.0, volume / 8.0))
