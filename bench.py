@@ -385,15 +385,19 @@ def main():
             if devs and world == 1 and name == args.workload:
                 f_count = min(e_count, 1 << 31)
                 f_ms = []
-                for _ in range(3):
-                    tmf = zb.zmc_scan_farm(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean[:f_count], h_err[:f_count],
-                                           devs, precision=w.precision, schedule=args.schedule, first_index=first,
-                                           count=f_count, batch_points=min(w.batch_points or f_count, max(1, f_count // (4 * len(devs)))),
-                                           consts=w.consts)
-                    f_ms.append(tmf["wall_ms"])
-                farm = {"devices": devs, "value": f_count * w.n_samples / (min(f_ms[1:]) * 1e-3), "unit": UNIT,
-                        "wall_ms": min(f_ms[1:]), "scanned_points": f_count, "n_batches": tmf["n_batches"],
-                        "batches_done": tmf["batches_done"], "busy_ms": tmf["busy_ms"]}
+                try:            # an extra record: a failure here (it has never run on more than one device) must not cost the line
+                    for _ in range(3):
+                        tmf = zb.zmc_scan_farm(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean[:f_count], h_err[:f_count],
+                                               devs, precision=w.precision, schedule=args.schedule, first_index=first,
+                                               count=f_count, batch_points=min(w.batch_points or f_count, max(1, f_count // (4 * len(devs)))),
+                                               consts=w.consts)
+                        f_ms.append(tmf["wall_ms"])
+                    farm = {"devices": devs, "value": f_count * w.n_samples / (min(f_ms[1:]) * 1e-3), "unit": UNIT,
+                            "wall_ms": min(f_ms[1:]), "scanned_points": f_count, "n_batches": tmf["n_batches"],
+                            "batches_done": tmf["batches_done"], "busy_ms": tmf["busy_ms"]}
+                except Exception as exc:        # noqa: BLE001 -- reported, not swallowed
+                    farm = {"devices": devs, "error": f"{type(exc).__name__}: {exc}"}
+                    torch.cuda.set_device(local_rank)
             del hplan, h_mean, h_err
 
         w_cyc, w_bound, w_res, w_add = w_min(w.name)

@@ -257,7 +257,7 @@ def pinned_empty(count: int, dtype, fill=None):
     for th in threads:
         th.join()
     rt = torch.cuda.cudart()
-    rc = rt.cudaHostRegister(arr.ctypes.data, nbytes, 0)
+    rc = rt.cudaHostRegister(arr.ctypes.data, nbytes, 1)          # cudaHostRegisterPortable: pinned for every device (farm)
     if int(rc) != 0:
         raise RuntimeError(f"cudaHostRegister of {nbytes} bytes failed: {rc}")
     t = torch.from_numpy(arr)
