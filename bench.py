@@ -377,7 +377,9 @@ def main():
                    "exposed_d2h_ms": float(np.mean([i["exposed_d2h_ms"] for i in e_infos])),
                    "n_batches": int(e_infos[-1]["n_batches"]), "host_out_pinned": int(e_infos[-1]["host_out_pinned"]),
                    "pin_seconds_not_timed": pin_s,
-                   "d2h_gbs": float(np.mean([i["d2h_bytes"] / max(i["d2h_ms"], 1e-9) * 1e-6 for i in e_infos]))}
+                   # results written by the kernel itself (host_out_pinned == 2: small one-batch scans) have no copy to rate
+                   "d2h_gbs": (float(np.mean([i["d2h_bytes"] / i["d2h_ms"] * 1e-6 for i in e_infos]))
+                               if all(i["d2h_ms"] > 0 for i in e_infos) else None)}
             launches += int(sum(i["gpu_launches"] for i in e_infos))
             # ---- NEXT-2: the single-node batch farm (host outputs, synchronous, host wall clock) -------------------
             devs = [int(d) for d in args.farm_devices.split(",")] if args.farm_devices else \

@@ -127,7 +127,9 @@ typedef struct zmc_timing {
     uint64_t h2d_bytes;      /* bytes this call copied host -> device (0 on a list-cache hit) */
     int32_t schedule;        /* the schedule actually used */
     int32_t host_out_pinned; /* HOST outputs: 1 = page-locked (copies overlap compute), 0 = pageable (cudaMemcpyAsync then runs
-                                synchronously on the host: no overlap, exposed_d2h_ms is the whole copy); -1 = device outputs */
+                                synchronously on the host: no overlap, exposed_d2h_ms is the whole copy); 2 = page-locked and
+                                small (one batch, <= 1 MiB of results): the kernel wrote them straight into host memory, no
+                                staging and no copy -- d2h_bytes counts them, d2h_ms stays 0; -1 = device outputs */
 } zmc_timing;
 
 /* What zmc_scan_farm did (the paper's allocation / evaluation view of Table 2). Host wall clock. */

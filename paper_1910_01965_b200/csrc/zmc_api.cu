@@ -543,17 +543,34 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     if (timing && h2d_bytes) { ZMC_CUDA(new_tev(&ev_h2d)); ZMC_CUDA(cudaEventRecord(ev_h2d, stream)); }
 
     // ---- H2: batches ----------------------------------------------------------------------------------
-    const bool host_out = o.out_location == ZMC_LOC_HOST;
+    bool host_out = o.out_location == ZMC_LOC_HOST;
     const size_t elem_out = p.out_f32 ? 4 : 8;
     const int64_t n_batches = zmc_batch_range(first, count, o.batch_points, -1, nullptr, nullptr);
     uint64_t batch_max = (o.batch_points == 0 || o.batch_points > count) ? count : o.batch_points;
+    // H8, small results: a one-batch scan whose results fit kDirectBytes and whose HOST buffers are page-locked and
+    // mapped is written by the kernel itself, straight into host memory (posted writes over PCIe / C2C): no staging
+    // buffer, no copy, no side stream.  For a 10^3-point grid the two copies and their events cost more than the kernel.
+    constexpr size_t kDirectBytes = 1u << 20;
+    bool direct = false;
+    uint64_t direct_bytes = 0;
     if (host_out) {
-        if (timing) {   // copies into pageable memory run synchronously on the host: report what the buffers are
-            cudaPointerAttributes pa;
-            const bool pinned = cudaPointerGetAttributes(&pa, out_mean) == cudaSuccess && pa.type == cudaMemoryTypeHost;
-            cudaGetLastError();
-            timing->host_out_pinned = pinned ? 1 : 0;
+        cudaPointerAttributes pa, pb, pc;
+        const bool pinned = cudaPointerGetAttributes(&pa, out_mean) == cudaSuccess && pa.type == cudaMemoryTypeHost;
+        cudaGetLastError();
+        if (timing) timing->host_out_pinned = pinned ? 1 : 0;   // copies into pageable memory run synchronously on the host
+        direct_bytes = count * (elem_out * 2 + (ad ? sizeof(uint32_t) : 0));
+        if (pinned && n_batches == 1 && direct_bytes <= kDirectBytes && pa.devicePointer &&
+            cudaPointerGetAttributes(&pb, out_stderr) == cudaSuccess && pb.type == cudaMemoryTypeHost && pb.devicePointer &&
+            (!ad || (cudaPointerGetAttributes(&pc, ad->out_n) == cudaSuccess && pc.type == cudaMemoryTypeHost && pc.devicePointer))) {
+            direct = true;
+            host_out = false;                                   // from here on: an ordinary one-batch scan into "device" pointers
+            out_mean = pa.devicePointer;
+            out_stderr = pb.devicePointer;
+            if (timing) timing->host_out_pinned = 2;            // 2 = pinned and written directly by the kernel
         }
+        cudaGetLastError();
+    }
+    if (host_out) {
         const size_t need = (size_t)batch_max * (elem_out * 2 + (ad ? sizeof(uint32_t) : 0));
         if (s->stage_cap < need) {
             for (int i = 0; i < 2; ++i) {          // wait for the copies still reading the old buffers, nothing else
@@ -573,7 +590,14 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     // indices and the grid size stay 32-bit.
     const uint64_t per_cta = schedule == ZMC_SCHED_THREAD ? kThreads
                            : (schedule == ZMC_SCHED_WARP || schedule == kSchedAdapt) ? kThreads / 32 : 1;
-    if (ad) { p.n_max = (uint32_t)ad->n_max; p.target = ad->target; p.out_n = ad->out_n; }
+    if (ad) {
+        p.n_max = (uint32_t)ad->n_max; p.target = ad->target; p.out_n = ad->out_n;
+        if (direct) {                                           // the device alias of the caller's host array
+            cudaPointerAttributes pc;
+            ZMC_CUDA(cudaPointerGetAttributes(&pc, ad->out_n));
+            p.out_n = static_cast<uint32_t*>(pc.devicePointer);
+        }
+    }
     constexpr uint64_t kMaxLaunchPoints = 1ull << 30;
 
     std::vector<TimedSpan> t_kernel, t_copy;
@@ -656,7 +680,7 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
         timing->exposed_d2h_ms = host_out ? (exposed > 0 ? exposed : 0.0) : 0.0;
         timing->n_batches = n_batches;
         timing->gpu_launches = launches;
-        timing->d2h_bytes = d2h_bytes;
+        timing->d2h_bytes = direct ? direct_bytes : d2h_bytes;     // direct: written by the kernel, inside kernel_ms
         timing->h2d_bytes = h2d_bytes;
     }
     return ZMC_OK;

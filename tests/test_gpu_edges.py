@@ -192,3 +192,40 @@ def test_pinned_empty_is_page_locked_host_memory_the_library_streams_into():
     assert small.is_pinned() and small.numel() == 1000
     del big, err, m, e
     gc.collect()                                                   # the registration is undone with the tensor
+
+
+def test_small_one_batch_host_scans_are_written_by_the_kernel_itself():
+    """H8, small results: one batch, <= 1 MiB, page-locked host buffers -> the kernel stores straight into host memory
+    (zmc_timing.host_out_pinned == 2, no copy); bit-identical to the device-output scan.  Larger, batched or pageable
+    outputs take the staged path."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(2, scale=[37, 29], n_samples=300)                       # 1073 points x 16 B
+    dm, de, _ = zb.scan_workload(w, host_out=False)
+    hm = torch.full((w.G + 64,), float("nan"), dtype=torch.float64).pin_memory()
+    he = torch.full((w.G + 64,), float("nan"), dtype=torch.float64).pin_memory()
+    _, _, tm = zb.scan_workload(w, out_mean=hm[32:32 + w.G], out_stderr=he[32:32 + w.G], host_out=True, batch_points=0, timing=True)
+    torch.cuda.synchronize()
+    assert tm["host_out_pinned"] == 2 and tm["d2h_bytes"] == 16 * w.G and tm["d2h_ms"] == 0 and tm["n_batches"] == 1
+    assert torch.equal(hm[32:32 + w.G], dm.cpu()) and torch.equal(he[32:32 + w.G], de.cpu())
+    assert bool(torch.isnan(hm[:32]).all()) and bool(torch.isnan(hm[32 + w.G:]).all())
+    # batched -> staged copies; pageable -> reported as such
+    _, _, tm = zb.scan_workload(w, out_mean=hm[32:32 + w.G], out_stderr=he[32:32 + w.G], host_out=True, batch_points=500, timing=True)
+    torch.cuda.synchronize()
+    assert tm["host_out_pinned"] == 1 and tm["n_batches"] == 3 and torch.equal(hm[32:32 + w.G], dm.cpu())
+    pm, pe = np.empty(w.G), np.empty(w.G)
+    import warnings
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore")
+        _, _, tm = zb.scan_workload(w, out_mean=pm, out_stderr=pe, host_out=True, batch_points=0, timing=True)
+    torch.cuda.synchronize()
+    assert tm["host_out_pinned"] == 0 and np.array_equal(pm, dm.cpu().numpy())
+    # the adaptive scan, out_n included
+    n_d = torch.zeros(w.G, dtype=torch.int32, device="cuda")
+    am, ae = torch.empty_like(dm), torch.empty_like(de)
+    zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, 256, 2048, 0.2, w.seed, am, ae, n_d)
+    n_h = torch.zeros(w.G, dtype=torch.int32).pin_memory()
+    tm = zb.zmc_scan_adaptive(w.integrand_id, w.bounds, w.lists, 256, 2048, 0.2, w.seed, hm[32:32 + w.G], he[32:32 + w.G], n_h, timing=True)
+    torch.cuda.synchronize()
+    assert tm["host_out_pinned"] == 2 and tm["d2h_bytes"] == 20 * w.G
+    assert torch.equal(n_h, n_d.cpu()) and torch.equal(hm[32:32 + w.G], am.cpu()) and torch.equal(he[32:32 + w.G], ae.cpu())
