@@ -365,7 +365,12 @@ def main():
             bp = w.batch_points or max(1, min(e_count, 1 << 22))      # stream in batches so copies overlap compute
             hplan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, h_mean, h_err, batch_points=bp,
                                 flags=zb.ZMC_OPT_FRESH_LISTS | shard_flags, **dict(common, count=e_count))
-            e_ms, e_infos = timed(lambda: hplan(stream, timing=True), e2e_steps, 1)
+            if tiny:        # as in the device arm: the timing report's synchronisation would be most of a sub-millisecond step
+                e2e_steps = max(e2e_steps, 10)
+                e_ms, _ = timed(lambda: hplan(stream), e2e_steps, 1)
+                _, e_infos = timed(lambda: hplan(stream, timing=True), min(e2e_steps, 3), 1)
+            else:
+                e_ms, e_infos = timed(lambda: hplan(stream, timing=True), e2e_steps, 1)
             e_evals_all = evals_all if e_count == count else e_count * w.n_samples * world
             e2e = {"value": e_evals_all / (e_ms / e2e_steps * 1e-3), "unit": UNIT,
                    "h2d_bytes_per_step": int(e_infos[-1]["h2d_bytes"]) * world,
@@ -380,7 +385,7 @@ def main():
                    # results written by the kernel itself (host_out_pinned == 2: small one-batch scans) have no copy to rate
                    "d2h_gbs": (float(np.mean([i["d2h_bytes"] / i["d2h_ms"] * 1e-6 for i in e_infos]))
                                if all(i["d2h_ms"] > 0 for i in e_infos) else None)}
-            launches += int(sum(i["gpu_launches"] for i in e_infos))
+            launches += int(sum(i["gpu_launches"] for i in e_infos)) + (int(e_infos[-1]["gpu_launches"]) * e2e_steps if tiny else 0)
             # ---- NEXT-2: the single-node batch farm (host outputs, synchronous, host wall clock) -------------------
             devs = [int(d) for d in args.farm_devices.split(",")] if args.farm_devices else \
                 (list(range(torch.cuda.device_count())) if torch.cuda.device_count() > 1 else [])
