@@ -15,7 +15,8 @@ def build(force: bool = False) -> str:
     import hashlib
     cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
            "-o", LIB + ".tmp", SRC, "-lm"]
-    stamp = hashlib.sha256(open(SRC, "rb").read() + " ".join(cmd).encode()).hexdigest()     # content, not file times
+    flags = " ".join(c for c in cmd if c not in (SRC, LIB + ".tmp"))                        # not the checkout's absolute paths
+    stamp = hashlib.sha256(open(SRC, "rb").read() + flags.encode()).hexdigest()             # content, not file times
     stamp_path = LIB + ".stamp"
     if not force and os.path.exists(LIB) and os.path.exists(stamp_path) and open(stamp_path).read().strip() == stamp:
         return LIB

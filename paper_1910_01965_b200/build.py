@@ -50,7 +50,8 @@ def _source_stamp(srcs, deps) -> str:
     """Hash of everything the library is built from.  File times are not trusted alone: a snapshot copied to another
     machine (gpurun) arrives with shuffled mtimes, and a rebuild there costs half a minute of GPU time."""
     import hashlib
-    h = hashlib.sha256(" ".join(FLAGS).encode())
+    # the flags without the checkout's absolute paths: the same sources at another path (the GPU box's scratch copy) are the same build
+    h = hashlib.sha256(" ".join("<include>" if f == INCLUDE else "<obj>" if f == OBJ else f for f in FLAGS).encode())
     for path in sorted(set(srcs + deps)):
         h.update(os.path.basename(path).encode())
         h.update(open(path, "rb").read())
