@@ -185,7 +185,11 @@ typedef struct zmc_integrand_info {
 ZMC_API zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                     uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream);
 
-/* Same, with options (may be NULL = defaults) and an optional timing report (may be NULL). */
+/* Same, with options (may be NULL = defaults) and an optional timing report (may be NULL).
+ * CUDA graphs: with DEVICE outputs, timing == NULL and value lists the library already holds on the device (any earlier
+ * call with the same lists), the call enqueues one kernel per launch and one event record on `stream` and nothing else,
+ * so it may be issued while `stream` is being captured.  The captured kernels read the library's cached copy of the
+ * lists: replay the graph before scanning with more than a few (7) other sets of value lists on that device. */
 ZMC_API zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                        uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream,
                        const zmc_options* opt, zmc_timing* timing);

@@ -229,3 +229,37 @@ def test_small_one_batch_host_scans_are_written_by_the_kernel_itself():
     torch.cuda.synchronize()
     assert tm["host_out_pinned"] == 2 and tm["d2h_bytes"] == 20 * w.G
     assert torch.equal(n_h, n_d.cpu()) and torch.equal(hm[32:32 + w.G], am.cpu()) and torch.equal(he[32:32 + w.G], ae.cpu())
+
+
+def test_a_scan_with_device_outputs_can_be_captured_into_a_cuda_graph():
+    """A scan into device memory whose value lists are already cached on the device enqueues one kernel and one event record
+    on the caller's stream (include/zmc.h, zmc_scan_ex): it can be captured into a CUDA graph and replayed, and ordinary
+    calls keep working afterwards (list uploads and evictions included)."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(2, scale=[41, 23], n_samples=500)
+    m = torch.zeros(w.G, dtype=torch.float64, device="cuda")
+    e = torch.zeros_like(m)
+    plan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, m, e, precision=w.precision, consts=w.consts)
+    s = torch.cuda.Stream()
+    plan(s)                                           # uploads the lists: the captured call must find them cached
+    s.synchronize()
+    ref_m, ref_e = m.clone(), e.clone()
+    m.zero_(); e.zero_()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        plan(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert not bool(m.any())                          # capture enqueued nothing
+    for _ in range(3):
+        m.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(m, ref_m) and torch.equal(e, ref_e)
+    for k in range(10):                               # more lists than cache slots: uploads and evictions after the capture
+        w2 = wl.config(2, scale=[41, 23], n_samples=500)
+        w2.lists[0] = wl.linspace(0.5, 5.0 + k, 41)
+        m2, e2, _ = zb.scan_workload(w2)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(m2).all())
