@@ -82,6 +82,19 @@ def test_cfg3_full_size_sampled():
     assert np.isfinite(mean).all() and np.isfinite(err).all()
 
 
+@pytest.mark.skipif(os.environ.get("ZMC_SKIP_DEEP_PARITY") == "1", reason="every point of cfg 2 and cfg 3 against the oracle: "
+                    "2.6e10 oracle evaluations, about two minutes on 16 host cores (BASELINE.md parity plan)")
+@pytest.mark.parametrize("k", [2, 3])
+def test_cfg2_cfg3_every_point(k):
+    """BASELINE.md "Parity coverage": configs 1-3 on the full grid.  cfg 1 is in the default suite above; these two cost
+    10^10 and 1.6*10^10 oracle evaluations (38 s and 90 s on the GPU box's 16 cores; ZMC_SKIP_DEEP_PARITY=1 leaves them out).  The oracle runs over the whole flat range in slices."""
+    w = wl.config(k)
+    mean, err, _ = gpu_scan(w)
+    step = 1 << 18
+    for first in range(0, w.G, step):
+        check(w, mean, err, np.arange(first, min(w.G, first + step), dtype=np.uint64))
+
+
 def test_cfg4_full_size_sampled():
     w = wl.config(4)
     mean, err, tm = gpu_scan(w)
