@@ -508,6 +508,18 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     }
     if (total > 0xFFFFFFFFull) return ZMC_ERR_GRID_TOO_LARGE;
     p.lists_total = (uint32_t)total;
+    // H3: reciprocals for the per-point digit extraction.  With s = max(2, ceil(log2 L)), P = 30 + s >= 32 and
+    // m = floor(2^P / L) + 1 < 2^32:  m L - 2^P = e in (0, L], so r m / 2^P = r / L + r e / (L 2^P) and the second term is
+    // below 1 / L for every r < 2^P / e, in particular for r < 2^30 (local indices of a launch): floor(r m / 2^P) = floor(r / L).
+    for (int i = 0; i < M; ++i) {
+        const uint64_t L = p.counts[i];
+        int sh = 2;
+        while ((1ull << sh) < L) ++sh;
+        p.div_m[i] = L > 1 ? (uint32_t)((1ull << (30 + sh)) / L + 1) : 0u;
+        p.div_s[i] = (uint32_t)(30 + sh - 32);
+    }
+    p.inv_n = 1.0 / (double)p.n;
+    p.nn1 = (double)(p.n - 1) * (double)p.n;
     const size_t elem_eval = f32e ? 4 : 8;
     // shared-memory staging pays off when a CTA serves many points (THREAD schedule) and the lists fit
     const size_t smem_bytes = (schedule == ZMC_SCHED_THREAD && total * elem_eval <= 48 * 1024) ? total * elem_eval : 0;

@@ -56,7 +56,8 @@ __device__ __forceinline__ void decode_point(const ScanParams& p, uint32_t local
     for (int i = ZMC_MAX_M - 1; i >= 1; --i) {
         if (i < M) {
             const uint32_t L = p.counts[i];
-            const uint32_t q = rest / L;
+            // rest / L without a division: rest < 2^30 (a launch's local index), so the host's 32-bit round-up reciprocal is exact
+            const uint32_t q = L == 1u ? rest : (__umulhi(rest, p.div_m[i]) >> p.div_s[i]);
             uint32_t d = p.base_digits[i] + (rest - q * L) + carry;
             carry = d >= L ? 1u : 0u;
             d -= carry ? L : 0u;
@@ -108,7 +109,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     const uint32_t n = p.n;
     const uint32_t n_full = n / S;                 // full groups; the last group may be clipped
     const uint32_t rem = n - n_full * S;
-    const double inv_n = 1.0 / (double)n;
+    const double inv_n = p.inv_n;                  // 1.0 / (double)n, divided once on the host (the same IEEE quotient)
 
     Fam fam;
     fam.setup(x, p);
@@ -203,7 +204,7 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
         double m2 = ::fma(-A * inv_n, A, B);
         m2 = m2 > 0.0 ? m2 : 0.0;
         const double mean = p.volume * mean_g;
-        const double serr = p.volume * sqrt(m2 / ((double)(n - 1) * (double)n));
+        const double serr = p.volume * sqrt(m2 / p.nn1);          // nn1 = (double)(n - 1) * (double)n
         const uint64_t o = p.out_off + local;
         if (p.out_f32) {
             static_cast<float*>(out_mean)[o] = (float)mean;

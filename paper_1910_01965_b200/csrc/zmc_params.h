@@ -20,6 +20,9 @@ struct ScanParams {
     uint32_t out_f32;             // 1: outputs are float
     uint32_t counts[ZMC_MAX_M];   // list lengths L_i
     uint32_t list_off[ZMC_MAX_M]; // offset of list i in `lists`
+    uint32_t div_m[ZMC_MAX_M];    // H3: floor(r / L_i) = umulhi(r, div_m[i]) >> div_s[i], exact for every r < 2^30 (host-computed
+    uint32_t div_s[ZMC_MAX_M];    //     round-up reciprocal, see fill_divisors in zmc_api.cu); unused where L_i == 1
+    double inv_n, nn1;            // H7: 1 / n and (n - 1) * n as doubles (the same IEEE operations the kernel would do per point)
     double a[ZMC_MAX_N], width[ZMC_MAX_N];   // box; in F32E mode already rounded to float (mirror, reading S5)
     double volume;                // prod_k width_k, k ascending
     // adaptive scan only (zmc_scan_adaptive, zmc_adapt_kernel): n is the first checkpoint
