@@ -263,3 +263,38 @@ def test_a_scan_with_device_outputs_can_be_captured_into_a_cuda_graph():
         m2, e2, _ = zb.scan_workload(w2)
     torch.cuda.synchronize()
     assert bool(torch.isfinite(m2).all())
+
+
+def test_decode_of_a_full_2_pow_30_point_launch_with_awkward_list_lengths():
+    """H3: the per-point digits come from host-computed reciprocals that are exact for local indices below 2^30 -- the most a
+    launch holds.  param_echo over a 1021 x 1031 x 1033 grid (1.09e9 points, prime lengths), first 2^30 points in ONE launch,
+    every digit of every point checked against integer arithmetic on the device; then a range that starts in the middle
+    (non-zero base digits, carries) and one with lists of length 1, 2, 3 and 65537."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+
+    def check(lengths, first, count):
+        lists = [np.arange(L, dtype=np.float64) for L in lengths]
+        strides = [int(np.prod(lengths[i + 1:])) for i in range(len(lengths))]
+        mean = torch.empty(count, dtype=torch.float32, device="cuda")
+        err = torch.empty(count, dtype=torch.float32, device="cuda")
+        for i, L in enumerate(lengths):
+            w = wl.Workload("echo", wl.D_PARAM_ECHO, np.array([0.0, 1.0]), lists, 2, 1, wl.PREC_F32E, np.array([float(i)]))
+            w.out_f32 = True
+            tm = zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, 2, 1, mean, err, None, precision=w.precision, schedule=1,
+                                first_index=first, count=count, consts=w.consts, timing=True)
+            assert tm["gpu_launches"] == (1 if count <= (1 << 30) else 2)
+            step = 1 << 26
+            for a in range(0, count, step):
+                t = torch.arange(first + a, first + min(count, a + step), dtype=torch.int64, device="cuda")
+                want = ((t // strides[i]) % L).to(torch.float32)
+                got = mean[a:a + len(t)]
+                assert torch.equal(got, want), (lengths, i, int((got != want).nonzero()[0]) + a + first)
+            assert not bool(err.any())
+        del mean, err
+        torch.cuda.empty_cache()
+
+    big = [1021, 1031, 1033]
+    check(big, 0, 1 << 30)
+    check(big, int(np.prod(big)) - (1 << 29) - 12345, (1 << 29) + 12345)          # up to the last point of the grid
+    check([3, 1, 65537, 2, 1], 0, 3 * 65537 * 2)
