@@ -16,6 +16,18 @@
 #pragma once
 #include "zmc_families.cuh"
 
+// 1/n and (n-1)n: taken from the parameter block (computed on the host) or recomputed per point.  The values are the same
+// IEEE results either way; what differs is the code ptxas generates AROUND them -- measured on B200: host values make the
+// built-in cfg 2 kernel 1.2 % faster (17.72 -> 17.50 ms), but the NVRTC-compiled user kernel of the same integrand 3.5 %
+// slower (19.13 -> 19.80 ms), so the run-time compiled kernels keep the per-point computation.
+#ifndef ZMC_FINALISE_FROM_HOST
+#ifdef __CUDACC_RTC__
+#define ZMC_FINALISE_FROM_HOST 0
+#else
+#define ZMC_FINALISE_FROM_HOST 1
+#endif
+#endif
+
 #ifndef ZMC_PIPELINE_F32
 #define ZMC_PIPELINE_F32 0      // measured with the two-buffer loop too: cfg3 -0.2 %, cfg4 -1.4 %, cfg5 -0.5 %
 #endif
@@ -109,7 +121,11 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
     const uint32_t n = p.n;
     const uint32_t n_full = n / S;                 // full groups; the last group may be clipped
     const uint32_t rem = n - n_full * S;
+#if ZMC_FINALISE_FROM_HOST
     const double inv_n = p.inv_n;                  // 1.0 / (double)n, divided once on the host (the same IEEE quotient)
+#else
+    const double inv_n = 1.0 / (double)n;
+#endif
 
     Fam fam;
     fam.setup(x, p);
@@ -204,7 +220,11 @@ zmc_scan_kernel(const __grid_constant__ ScanParams p, void* __restrict__ out_mea
         double m2 = ::fma(-A * inv_n, A, B);
         m2 = m2 > 0.0 ? m2 : 0.0;
         const double mean = p.volume * mean_g;
+#if ZMC_FINALISE_FROM_HOST
         const double serr = p.volume * sqrt(m2 / p.nn1);          // nn1 = (double)(n - 1) * (double)n
+#else
+        const double serr = p.volume * sqrt(m2 / ((double)(n - 1) * (double)n));
+#endif
         const uint64_t o = p.out_off + local;
         if (p.out_f32) {
             static_cast<float*>(out_mean)[o] = (float)mean;
