@@ -50,6 +50,7 @@ extern "C" {
 #define ZMC_MAX_M 8         /* parameters */
 #define ZMC_MAX_CONSTS 8    /* family constants */
 #define ZMC_MAX_FARM_DEVICES 16   /* devices of one node in zmc_scan_farm */
+#define ZMC_NOALLOC_MAX_LIST_VALUES 4096   /* zmc_scan_noalloc: most list entries (all M lists together) one call may pass */
 
 typedef enum zmc_status {
     ZMC_OK = 0,
@@ -60,7 +61,8 @@ typedef enum zmc_status {
     ZMC_ERR_GRID_TOO_LARGE = 4,    /* prod(count) > 2^48, or one list longer than 2^31-1 */
     ZMC_ERR_OUT_OF_MEMORY = 5,
     ZMC_ERR_CUDA = 6,              /* see zmc_last_cuda_error() */
-    ZMC_ERR_COMPILE = 7            /* zmc_register_integrand: NVRTC missing or the body does not compile; see zmc_last_compile_log() */
+    ZMC_ERR_COMPILE = 7,           /* zmc_register_integrand: NVRTC missing or the body does not compile; see zmc_last_compile_log() */
+    ZMC_ERR_NOALLOC_LIMIT = 8      /* zmc_scan_noalloc only: the value lists hold more than ZMC_NOALLOC_MAX_LIST_VALUES entries in total */
 } zmc_status;
 
 /* Integrand families g(y; x), SURVEY.md 8(c) S7 / BASELINE.json configs.  y_k is 0-based. */
@@ -193,6 +195,36 @@ ZMC_API zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M
 ZMC_API zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                        uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream,
                        const zmc_options* opt, zmc_timing* timing);
+
+/*
+ * zmc_scan_noalloc -- zmc_scan_ex for callers that must not allocate GPU memory.
+ * Some programs cannot let a library call cudaMalloc / cudaFree on their behalf: a server or framework that gave all
+ * device memory to its own pool at start-up (a hidden allocation can turn into the owner's out-of-memory error later), a
+ * latency-critical loop (both calls take a driver lock and may synchronise the whole device, stalling every stream), or a
+ * deployment whose buffer plan was fixed in advance.  zmc_scan_ex keeps its device copy of the value lists in memory it
+ * allocates on demand; this entry point keeps it in a fixed array that is part of the library image instead
+ * (ZMC_NOALLOC_MAX_LIST_VALUES doubles = 32 KiB on every GPU that loads the library, held until the process exits).
+ * It calls no cudaMalloc, cudaFree, cudaMallocHost, stream / event creation or other allocating routine: it only
+ * launches kernels on `stream` (the list values travel as kernel arguments, so `lists` is free again on return).
+ *   Arguments   as zmc_scan_ex, without `timing`.  out_mean / out_stderr are DEVICE memory owned by the caller
+ *               (opt->out_location must be ZMC_LOC_DEVICE; opt may be NULL).  Built-in families only (ids < 1000).
+ *               opt->batch_points is ignored (batches exist to stream results to the host); ZMC_OPT_FRESH_LISTS has no
+ *               effect (the lists are written into the array by every call).
+ *   Results     bit-identical to zmc_scan_ex with the same arguments and schedule (tests/test_zz_no_alloc.py).
+ *   Errors      those of zmc_scan_ex, detected before anything is enqueued, plus ZMC_ERR_NOALLOC_LIMIT when
+ *               sum_i lists[i].count > ZMC_NOALLOC_MAX_LIST_VALUES (use zmc_scan_ex for longer lists).
+ *   First call  the first call on each device looks up the array's device address (the device must be current, as
+ *               for every call) and loads the kernels it launches; make that first call during start-up, before any
+ *               stream capture is begun on that device.
+ *   Sharing     every call on a device uses the same array and finds in it whatever the previous call left; each call
+ *               overwrites the entries it reads, so nothing has to be cleared between calls.  Calls issued one after
+ *               another on ONE stream are ordered by the stream.  Calls whose GPU work may overlap -- two streams, or
+ *               two host threads on the same device -- race on the array and give undefined results: serialise them.
+ *               (zmc_scan_ex does not use this array and may run concurrently.)
+ */
+ZMC_API zmc_status zmc_scan_noalloc(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
+                            uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream,
+                            const zmc_options* opt);
 
 /* Pure host helpers (no GPU needed). */
 ZMC_API int zmc_integrand_count(void);

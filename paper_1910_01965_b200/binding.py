@@ -20,6 +20,8 @@ LIB_PATH = os.path.join(_HERE, "libzmc.so")
 ZMC_OK, ZMC_ERR_INVALID_ARG, ZMC_ERR_UNKNOWN_INTEGRAND, ZMC_ERR_SHAPE_MISMATCH = 0, 1, 2, 3
 ZMC_ERR_GRID_TOO_LARGE, ZMC_ERR_OUT_OF_MEMORY, ZMC_ERR_CUDA = 4, 5, 6
 ZMC_ERR_COMPILE = 7
+ZMC_ERR_NOALLOC_LIMIT = 8
+ZMC_NOALLOC_MAX_LIST_VALUES = 4096
 ZMC_PREC_F64, ZMC_PREC_F32E = 0, 1
 ZMC_OUT_F64, ZMC_OUT_F32 = 0, 1
 ZMC_LOC_DEVICE, ZMC_LOC_HOST = 0, 1
@@ -33,7 +35,7 @@ EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info
            "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown",
            "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm", "zmc_scan_adaptive",
            "zmc_pick_schedule_ex", "zmc_register_integrand_ex", "zmc_unregister_integrand", "zmc_scan_farm_adaptive",
-           "zmc_measure_pipes"]
+           "zmc_measure_pipes", "zmc_scan_noalloc"]
 
 
 class zmc_param_list(ctypes.Structure):
@@ -120,6 +122,8 @@ def load():
     lib.zmc_scan.restype = ctypes.c_int
     lib.zmc_scan_ex.argtypes = scan_args + [P(zmc_options), P(zmc_timing)]
     lib.zmc_scan_ex.restype = ctypes.c_int
+    lib.zmc_scan_noalloc.argtypes = scan_args + [P(zmc_options)]
+    lib.zmc_scan_noalloc.restype = ctypes.c_int
     lib.zmc_integrand_count.restype = ctypes.c_int
     lib.zmc_integrand_info_at.argtypes = [ctypes.c_int, P(zmc_integrand_info)]
     lib.zmc_integrand_info_by_id.argtypes = [ctypes.c_int, P(zmc_integrand_info)]
@@ -318,6 +322,27 @@ def zmc_scan_ex(integrand_id: int, bounds, lists, n_samples: int, seed: int, out
                               ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(_stream_handle(stream)),
                               ctypes.byref(o), ctypes.byref(tm) if timing else None))
     return tm.as_dict() if timing else None
+
+
+def zmc_scan_noalloc(integrand_id: int, bounds, lists, n_samples: int, seed: int, out_mean, out_stderr, stream=None, *,
+                     precision: int = ZMC_PREC_F64, schedule: int = ZMC_SCHED_AUTO,
+                     fast_math: int = ZMC_FAST_MATH_DEFAULT, first_index: int = 0, count: int = 0, consts=None,
+                     flags: int = 0) -> None:
+    """include/zmc.h zmc_scan_noalloc: the scan for callers that must not allocate GPU memory (a process whose device
+    memory all belongs to its own pool, a latency-critical loop, a fixed buffer plan).  The library's copy of the value
+    lists lives in a fixed 32 KiB array inside libzmc.so instead of cudaMalloc'ed memory, so at most
+    ZMC_NOALLOC_MAX_LIST_VALUES list entries in total (else ZmcError with status ZMC_ERR_NOALLOC_LIMIT).  Outputs are
+    CUDA tensors the caller allocated; built-in families only.  Overlapping calls on one device race on that array --
+    issue them on one stream.  Same results, bit for bit, as zmc_scan_ex."""
+    m = _Marshalled(bounds, lists, consts)
+    pm, dm, lm = _tensor_ptr(out_mean)
+    pe, de, le = _tensor_ptr(out_stderr)
+    if (dm, lm) != (de, le):
+        raise ZmcError(ZMC_ERR_INVALID_ARG, "out_mean and out_stderr must share dtype and location")
+    o = _make_options(m, precision, dm, lm, schedule, fast_math, 0, first_index, count, flags)
+    _check(load().zmc_scan_noalloc(integrand_id, m.N, m.bounds_ptr(), m.M, m.c_lists, n_samples, seed,
+                                   ctypes.c_void_p(pm), ctypes.c_void_p(pe), ctypes.c_void_p(_stream_handle(stream)),
+                                   ctypes.byref(o)))
 
 
 def zmc_validate(integrand_id: int, bounds, lists, n_samples: int, *, precision: int = ZMC_PREC_F64,

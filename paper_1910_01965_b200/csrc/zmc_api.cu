@@ -351,6 +351,7 @@ const char* zmc_status_string(zmc_status s) {
         case ZMC_ERR_OUT_OF_MEMORY: return "out of memory";
         case ZMC_ERR_CUDA: return "CUDA error (see zmc_last_cuda_error)";
         case ZMC_ERR_COMPILE: return "user integrand did not compile (see zmc_last_compile_log)";
+        case ZMC_ERR_NOALLOC_LIMIT: return "value lists exceed ZMC_NOALLOC_MAX_LIST_VALUES entries in total (zmc_scan_noalloc has a fixed buffer; use zmc_scan_ex)";
     }
     return "unknown status";
 }
