@@ -4,8 +4,8 @@ anywhere in it -- a dropped term, a wrong sign or index, a transposed operand --
 Each mutation below is one such mistake, applied to a scratch copy of oracle/zmc_oracle.c; the copy is built on its own
 (ZMC_ORACLE_SRC / ZMC_ORACLE_LIB, oracle/build.py) and the oracle's pin tests are run against it in a subprocess.  The audit
 passes when every mutated oracle turns at least one pin test red.  The first two are the ones the round-1 review found
-passing (c5's factor, c4's parameter assignment).  By default a handful run (the CPU suite stays short);
-ZMC_MUTATION_AUDIT=1 runs them all (about three minutes).  Nothing here touches the CUDA path.
+passing (c5's factor, c4's parameter assignment).  By default the first eight run (the CPU suite stays short);
+ZMC_MUTATION_AUDIT=1 runs all 24 (about four minutes).  Nothing here touches the CUDA path.
 """
 import os
 import subprocess
@@ -23,6 +23,13 @@ MUTATIONS = [
     ("c4: x3 and x4 swapped", "(k < 2) ? x[1] : (k < 4) ? x[2] : x[3]", "(k < 2) ? x[1] : (k < 4) ? x[3] : x[2]"),
     ("stream: lanes of a block taken in reverse order", "return r[q & 3];", "return r[3 - (q & 3)];"),
     ("estimator: biased variance (n instead of n - 1)", "ss / (long double)(p->n - 1)", "ss / (long double)(p->n)"),
+    # reading S5, the four single-line mistakes the round-2 review found passing (pinned by the S5_BOX cases of test_oracle_pins.py)
+    ("sample map: width rounded as float(b) - float(a) instead of float(b - a)",
+     "width[k] = mirror(p->bounds[2 * k + 1] - p->bounds[2 * k], p->mode);",
+     "width[k] = mirror(p->bounds[2 * k + 1], p->mode) - mirror(p->bounds[2 * k], p->mode);"),
+    ("sample map: a_k not rounded in mirror mode", "a[k] = mirror(p->bounds[2 * k], p->mode);", "a[k] = p->bounds[2 * k];"),
+    ("family constants not rounded in mirror mode", "cst[c] = mirror(p->consts[c], p->mode);", "cst[c] = p->consts[c];"),
+    ("sample map: u * width + a without the fused multiply-add", "y[k] = fma(u, width[k], a[k]);", "y[k] = u * width[k] + a[k];"),
     # ---- the rest run with ZMC_MUTATION_AUDIT=1 ----
     ("c5: phase coefficients permuted", "x[1] * y[0] + x[2] * y[1] + x[3] * y[2]", "x[2] * y[0] + x[1] * y[1] + x[3] * y[2]"),
     ("c5: a y_k dropped from the factor", "(1.0 + x[4] * y[0] * y[1] * y[2])", "(1.0 + x[4] * y[0] * y[1])"),
@@ -41,7 +48,7 @@ MUTATIONS = [
     ("estimator: stderr without the volume", "(long double)V * sqrtl(var / (long double)p->n)", "sqrtl(var / (long double)p->n)"),
     ("decode: first list fastest", "for (int i = p->M - 1; i >= 0; --i) {\n        uint64_t L", "for (int i = 0; i < p->M; ++i) {\n        uint64_t L"),
 ]
-N_DEFAULT = 4
+N_DEFAULT = 8
 FULL = os.environ.get("ZMC_MUTATION_AUDIT") == "1"
 
 

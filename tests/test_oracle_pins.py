@@ -125,6 +125,7 @@ def test_const_one_gives_volume_and_zero_stderr():
 
 
 # ---- T5 -----------------------------------------------------------------------------------
+S5_BOX = [0.1, 0.7, -0.3, 1.9]
 BF_CASES = [
     # fid, bounds, lists, n, consts, bit_exact
     (wl.D_POLY, [0.0, 1.0, -1.0, 2.0], [[1.0, 2.0], [0.5, 1.5, 2.5]], 5, (), True),
@@ -141,7 +142,41 @@ BF_CASES = [
      [[1.0, 2.5], [0.2], [0.45, 0.7], [0.9, 0.1]], 5, (), False),
     (wl.C5_DAMPED_COS, [-1.0, 1.0, -1.0, 1.0, -1.0, 1.0], [[0.1, 1.3], [0.7], [2.9, 1.1], [4.0], [3.7, 0.4]], 6, (), False),
     (wl.C5_DAMPED_COS, [0.0, 1.0, -0.5, 1.0, 0.25, 2.0], [[0.3], [1.7], [0.6], [2.2], [1.9, -2.5]], 7, (), False),
+    # reading S5 (Eq. 1 is silent on the sample map, so the reading is the definition):
+    # boxes and constants that are NOT exactly representable in float and whose widths are not short dyadics.  F64 mode:
+    # u * width needs more than 53 bits, so fma(u, width, a) and the unfused u * width + a differ in the last bit of many
+    # samples (bit-exact families).  Mirror mode: float(a_k) != a_k, float(b - a) != float(b) - float(a) and
+    # float(u) != u (asserted in test_s5_cases_exercise_every_rounding_site below), so leaving any of them unrounded,
+    # or rounding the width the other way, moves every sample by ~1e-8.
+    (wl.D_POLY, S5_BOX, [[1.0, 2.0], [0.5, 1.5, 2.5]], 9, (), True),
+    (wl.D_LIN_Y, S5_BOX, [[1.0, 2.0], [0.5, 1.5]], 9, (0.0,), True),
+    (wl.D_LIN_Y, S5_BOX, [[1.0, 2.0], [0.5, 1.5]], 9, (1.0,), True),
+    (wl.C3_OSCILLATORY, S5_BOX, [[0.1, 3.0], [1.0, 2.0], [0.3, 0.7]], 6, (0.6,), False),
 ]
+
+
+def test_s5_cases_exercise_every_rounding_site():
+    """The S5 cases above only pin what they claim if the roundings they are meant to catch are not the identity."""
+    import struct
+
+    def f32(v):
+        return struct.unpack("f", struct.pack("f", v))[0]
+
+    for k in range(len(S5_BOX) // 2):
+        a, b = S5_BOX[2 * k], S5_BOX[2 * k + 1]
+        assert f32(a) != a                                   # "a_k not rounded in mirror mode" changes y
+        assert f32(b - a) != f32(b) - f32(a)                 # "width = float(b) - float(a)" changes y
+        assert f32(b - a) != b - a
+    assert f32(0.6) != 0.6                                   # "consts not rounded in mirror mode" changes c3's phase
+    # F64 mode: the product u * width is inexact for these widths, so fused and unfused sample maps differ somewhere
+    differ = 0
+    for t in range(4):
+        for q in range(18):
+            u = bf.uniform_exact(bf.word(3, t, q))
+            k = q % 2
+            a, w = S5_BOX[2 * k], S5_BOX[2 * k + 1] - S5_BOX[2 * k]
+            differ += bf._fma(float(u), w, a) != float(u) * w + a
+    assert differ >= 10
 
 
 @pytest.mark.parametrize("case", BF_CASES)
@@ -158,7 +193,9 @@ def test_brute_force_tiny_grids(case, mirror):
         assert rc == 0
         if exact:
             assert list(gs) == g                     # every sample value bit-exact
-            assert abs(mean[t] - m) <= 2e-16 * abs(m)
+            # the enumerator rounds three times in double (fsum, / n, * V -- V is inexact for S5_BOX), the oracle once from
+            # long double (reading S6): up to 1.5 ulp = 3.4e-16 apart
+            assert abs(mean[t] - m) <= 4e-16 * abs(m)
             assert abs(err[t] - e) <= 1e-15 * abs(e) + 1e-300
         else:
             assert np.allclose(gs, g, rtol=0, atol=1e-15)
