@@ -189,9 +189,13 @@ ZMC_API zmc_status zmc_scan(int integrand_id, int N, const double* bounds, int M
 
 /* Same, with options (may be NULL = defaults) and an optional timing report (may be NULL).
  * CUDA graphs: with DEVICE outputs, timing == NULL and value lists the library already holds on the device (any earlier
- * call with the same lists), the call enqueues one kernel per launch and one event record on `stream` and nothing else,
- * so it may be issued while `stream` is being captured.  The captured kernels read the library's cached copy of the
- * lists: replay the graph before scanning with more than a few (7) other sets of value lists on that device. */
+ * call with the same lists, not yet displaced by 8 other sets), the call enqueues one kernel per launch on `stream` and
+ * nothing else, so it may be issued while `stream` is being captured.  The captured kernels read the library's cached
+ * copy of the lists; the library therefore keeps that copy untouched -- never evicted, overwritten or freed -- until
+ * zmc_shutdown, so the graph can be replayed at any later time, whatever is scanned in between.  At most 7 different
+ * sets of value lists can be held for graphs per device.  A call issued during capture that cannot be captured (lists
+ * not cached, an 8th set, host outputs, timing != NULL) returns ZMC_ERR_CUDA with zmc_last_cuda_error() =
+ * cudaErrorStreamCaptureUnsupported (900) and enqueues nothing. */
 ZMC_API zmc_status zmc_scan_ex(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                        uint64_t n_samples, uint64_t seed, void* out_mean, void* out_stderr, void* stream,
                        const zmc_options* opt, zmc_timing* timing);
@@ -237,7 +241,9 @@ ZMC_API const char* zmc_version(void);
 ZMC_API zmc_status zmc_validate(int integrand_id, int N, const double* bounds, int M, const zmc_param_list* lists,
                         uint64_t n_samples, const zmc_options* opt, uint64_t* grid_points);
 /* The schedule AUTO would pick for `count` points of `n_samples` samples in N dimensions (fp64 path; _ex: either
- * precision -- the fp32-evaluate kernels keep more threads resident, so their thresholds are higher). */
+ * precision -- the fp32-evaluate kernels keep more threads resident, so their thresholds are higher).  The thresholds
+ * scale with the SM count of the CURRENT device (148 if none is visible).  The schedule fixes the order of the sums,
+ * hence the last bits of the results: for bit-identical results across different GPUs pass an explicit schedule. */
 ZMC_API int zmc_pick_schedule(uint64_t count, uint64_t n_samples, int N);
 ZMC_API int zmc_pick_schedule_ex(uint64_t count, uint64_t n_samples, int N, int precision);
 /* Batch b of a range cut into batches of batch_points: writes its (first, count). Returns the number of batches. */
@@ -297,14 +303,18 @@ ZMC_API zmc_status zmc_scan_farm_adaptive(int integrand_id, int N, const double*
  * the MUFU forms after an exact range reduction (absolute error ~1e-6) and NVRTC --use_fast_math for the rest of the body.
  * Plain sin()/cos()/exp() work too (libdevice), at about half the speed in fp64.
  * Compiled integrands are CACHED by the hash of (body, N, M, n_consts, flags): registering the same integrand again costs
- * microseconds and returns the same id.  Host strings are copied.  ZMC_ERR_COMPILE: libnvrtc.so.12 not found or compilation
+ * microseconds and returns the same id (with the first registrant's name), counted: see zmc_unregister_integrand.  Host strings are copied.  ZMC_ERR_COMPILE: libnvrtc.so.12 not found or compilation
  * failed (log below); ZMC_ERR_CUDA: compiled, but the code could not be loaded (no usable device).  zmc_options.fast_math is
  * ignored for user integrands (use ZMC_USER_FAST_MATH at registration).
  */
 ZMC_API zmc_status zmc_register_integrand(const char* name, const char* body, int N, int M, int n_consts, int* integrand_id);
 ZMC_API zmc_status zmc_register_integrand_ex(const char* name, const char* body, int N, int M, int n_consts, int flags,
                                      int* integrand_id);
-/* Forget a user integrand and unload its code.  No scan using it may be in flight.  ZMC_ERR_UNKNOWN_INTEGRAND if not registered. */
+/* Give up one registration of a user integrand.  An id handed out more than once (the same integrand registered again,
+ * possibly by another part of the program) stays valid until it has been unregistered as many times as it was registered;
+ * the last call forgets the id and unloads the code.  Scans already enqueued are safe: the library waits for the devices
+ * that are running the integrand's kernels before unloading, and a scan call in progress on another thread keeps the code
+ * loaded until it returns.  ZMC_ERR_UNKNOWN_INTEGRAND if the id is not (or no longer) registered. */
 ZMC_API zmc_status zmc_unregister_integrand(int integrand_id);
 ZMC_API const char* zmc_last_compile_log(void);   /* NVRTC log of the last zmc_register_integrand on this thread */
 /*

@@ -4,6 +4,7 @@
 // PAPER.md:65 "we cut the parameter grid into several batches. Each batch is fed into one GPU
 // device for evaluation"; PAPER.md:85, :132-140 report HToD, DToH and GPU evaluation time
 // separately -- zmc_timing keeps that split.  There is no CPU fallback anywhere in this file.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -63,7 +64,7 @@ namespace {
 const zmc_integrand_info* find_family(int id, zmc_integrand_info* storage) {
     for (int i = 0; i < kNumFamilies; ++i)
         if (kFamilies[i].id == id) return &kFamilies[i];
-    if (const UserIntegrand* u = find_user_integrand(id)) {
+    if (const std::shared_ptr<const UserIntegrand> u = find_user_integrand(id)) {
         *storage = zmc_integrand_info{u->id, u->name.c_str(), u->N, u->N, u->M, u->M, u->n_consts, 0};
         return storage;
     }
@@ -162,7 +163,10 @@ struct ListSlot {
     cudaEvent_t uploaded = nullptr;  // the H2D copy into `dev`
     cudaStream_t last_stream = nullptr;
     bool multi_stream = false;   // read from more than one stream since the upload: `done` does not cover all readers
+    bool upload_pending = false; // `uploaded` has not been seen complete yet
     bool used = false;
+    bool captured = false;       // a CUDA graph holds `dev` in a kernel node (the call was issued during stream capture): the
+                                 // slot is never evicted, overwritten or reallocated again until zmc_shutdown
     uint64_t last_use = 0;
 };
 struct DeviceScratch {
@@ -250,7 +254,16 @@ bool same_lists(const ListSlot& c, int M, const zmc_param_list* lists, const uin
 // H1: the device copy of the concatenated lists -- a cache hit enqueues nothing, a miss uploads through the slot's
 // pinned buffer on `stream`.  *h2d_bytes = bytes actually copied by this call.
 zmc_status stage_lists(DeviceScratch* s, int M, const zmc_param_list* lists, const uint32_t* list_off, size_t total,
-                       bool fresh, cudaStream_t stream, ListSlot** out, size_t* h2d_bytes) {
+                       bool fresh, cudaStream_t stream, ListSlot** out, size_t* h2d_bytes, bool* capturing_out) {
+    // A call issued while `stream` is being captured bakes the slot's device pointer into the graph's kernel nodes, and the
+    // graph may be replayed at any later time: such a slot is marked `captured` and stays as it is until zmc_shutdown.
+    // A captured call cannot upload (the copy and its allocations would become graph nodes reading the library's pinned
+    // buffer at replay time), so its lists must already be cached -- otherwise it is refused before anything is enqueued.
+    cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
+    ZMC_CUDA(cudaStreamIsCapturing(stream, &cap_status));
+    const bool capturing = cap_status != cudaStreamCaptureStatusNone;
+    *capturing_out = capturing;
+    if (capturing) fresh = false;
     ListSlot* hit = nullptr;
     uint64_t h = 0;
     if (!fresh) {
@@ -266,18 +279,40 @@ zmc_status stage_lists(DeviceScratch* s, int M, const zmc_param_list* lists, con
             if (s->ring[i].hash == h && same_lists(s->ring[i], M, lists, list_off, total)) hit = &s->ring[i];
     }
     *h2d_bytes = 0;
+    if (capturing) {
+        int n_captured = 0;
+        for (int i = 0; i < kRing; ++i) n_captured += s->ring[i].captured ? 1 : 0;
+        // not cached, or the last slot ordinary calls could still use: refuse (cudaErrorStreamCaptureUnsupported)
+        if (!hit || (!hit->captured && n_captured >= kRing - 1)) return cuda_fail(cudaErrorStreamCaptureUnsupported);
+        hit->captured = true;
+    }
     if (hit) {
-        if (hit->last_stream != stream) {      // another stream uploaded it: order this stream's kernels after that copy
+        // Order this stream's kernels after the upload unless it is known to be behind them already.  The stream HANDLE is
+        // not proof: a destroyed stream's handle is reused by the next one created (zmc_scan_farm does that on every call),
+        // so the same-handle shortcut is taken only while the upload has visibly completed or the slot has never been
+        // read from another handle since.  (No event query during capture: not permitted there.)
+        bool ordered = hit->last_stream == stream && !hit->multi_stream;
+        if (ordered && !capturing && hit->upload_pending) {
+            if (cudaEventQuery(hit->uploaded) == cudaSuccess) hit->upload_pending = false;
+            else { cudaGetLastError(); ordered = false; }
+        }
+        if (!ordered) {
             ZMC_CUDA(cudaStreamWaitEvent(stream, hit->uploaded, 0));
-            hit->multi_stream = true;
+            if (hit->last_stream != stream) hit->multi_stream = true;
         }
     } else {
-        hit = &s->ring[0];                      // victim: a free slot if there is one, else the least recently used
-        for (int i = 1; i < kRing && hit->used; ++i)
-            if (!s->ring[i].used || s->ring[i].last_use < hit->last_use) hit = &s->ring[i];
+        hit = nullptr;                          // victim: a free slot if there is one, else the least recently used; never a captured one
+        for (int i = 0; i < kRing; ++i) {
+            ListSlot* c = &s->ring[i];
+            if (c->captured) continue;
+            if (!hit || (hit->used && (!c->used || c->last_use < hit->last_use))) hit = c;
+        }
+        if (!hit) return ZMC_ERR_OUT_OF_MEMORY;  // cannot happen: at most kRing - 1 slots are ever captured
         if (hit->used) {                        // evict: every kernel that reads the old content must have finished
             if (hit->multi_stream) ZMC_CUDA(cudaDeviceSynchronize());
             else ZMC_CUDA(cudaEventSynchronize(hit->done));
+            // a scan that failed after its upload never recorded `done`: the copy out of `host` may still be in flight
+            if (hit->upload_pending) ZMC_CUDA(cudaEventSynchronize(hit->uploaded));
         }
         hit->used = false;
         if (hit->cap < total) {
@@ -292,7 +327,7 @@ zmc_status stage_lists(DeviceScratch* s, int M, const zmc_param_list* lists, con
             std::memcpy(hit->host + list_off[l], lists[l].values, (size_t)lists[l].count * sizeof(double));
         ZMC_CUDA(cudaMemcpyAsync(hit->dev, hit->host, total * sizeof(double), cudaMemcpyHostToDevice, stream));
         ZMC_CUDA(cudaEventRecord(hit->uploaded, stream));
-        hit->hash = h; hit->total = total; hit->multi_stream = false; hit->used = true;
+        hit->hash = h; hit->total = total; hit->multi_stream = false; hit->used = true; hit->upload_pending = true;
         *h2d_bytes = total * sizeof(double);
     }
     hit->last_stream = stream;
@@ -369,27 +404,25 @@ zmc_status zmc_validate(int integrand_id, int N, const double* bounds, int M, co
 }
 
 // H6 schedule choice.  R = threads the device keeps resident: the fp64 kernels are launch-bounded to 3 CTAs of 256
-// per SM, the fp32-evaluate ones to 4 (zmc_kernel.cuh); the SM count is the current device's (148 on a B200, also the
-// fallback when no device is visible).  THREAD needs >= 8 rounds of R (measured on cfg 2, 8.8 rounds: 2.8 % faster
+// per SM, the fp32-evaluate ones to 4 (zmc_kernel.cuh); the SM count is the current device's (looked up once per device; 148, a
+// B200's, while no device is visible).  THREAD needs >= 8 rounds of R (measured on cfg 2, 8.8 rounds: 2.8 % faster
 // than WARP because rounds 1-2 of Philox run on the uniform datapath); WARP needs 2 rounds of R/32 resident warps
 // (measured on B200 for the cfg 1-3 families with 2000-16000 points x 5000-50000 samples: below that the finer
 // granularity of one CTA per point wins by up to 20 %, above it WARP by 5-15 % -- one shuffle tree instead of a tree,
 // a barrier and a second tree per point); else CTA.  A point with few sample groups cannot feed 32 / 256 lanes, so
 // small n falls back to fewer lanes.
-static int cached_sm_count() {
-    static int sms = [] {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
-            cudaGetLastError();
-            return 148;
-        }
-        return n;
-    }();
-    return sms;
+static int current_sm_count() {     // of the CURRENT device, remembered per device; nothing is latched while no device answers
+    static std::atomic<int> known[kMaxDevices];
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return 148; }
+    if ((n = known[dev].load(std::memory_order_relaxed)) > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) { cudaGetLastError(); return 148; }
+    known[dev].store(n, std::memory_order_relaxed);
+    return n;
 }
 
 int zmc_pick_schedule_ex(uint64_t count, uint64_t n_samples, int N, int precision) {
-    const uint64_t resident = (uint64_t)cached_sm_count() * (precision == ZMC_PREC_F32E ? 1024ull : 768ull);
+    const uint64_t resident = (uint64_t)current_sm_count() * (precision == ZMC_PREC_F32E ? 1024ull : 768ull);
     const int g4 = (N % 4 == 0) ? 4 : (N % 2 == 0) ? 2 : 1;
     const uint64_t groups = n_samples / (uint64_t)(4 / g4) + 1;
     if (count >= 8 * resident || groups < 4 * 32) return ZMC_SCHED_THREAD;
@@ -463,7 +496,7 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     const int fast = f32e ? (o.fast_math == ZMC_FAST_MATH_OFF ? 0 : 1) : 0;
     const int schedule = ad ? (int)kSchedAdapt
                        : o.schedule == ZMC_SCHED_AUTO ? zmc_pick_schedule_ex(count, n_samples, N, o.precision) : o.schedule;
-    const UserIntegrand* user = integrand_id >= kFirstUserId ? find_user_integrand(integrand_id) : nullptr;
+    const std::shared_ptr<const UserIntegrand> user = integrand_id >= kFirstUserId ? find_user_integrand(integrand_id) : nullptr;   // held for the whole call
     const KernelEntry* kern = user ? nullptr : find_kernel(integrand_id, N, o.precision, fast, schedule);
     if (!kern && !user) return ZMC_ERR_UNKNOWN_INTEGRAND;
     if (timing) { timing->schedule = ad ? (int)ZMC_SCHED_WARP : schedule; timing->host_out_pinned = -1; }
@@ -476,6 +509,12 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     DeviceScratch* s = nullptr;
     st = get_scratch(dev, &s);
     if (st != ZMC_OK) return st;
+
+    if (timing || o.out_location == ZMC_LOC_HOST) {     // these synchronise / copy on a side stream: not capturable, say so up front
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        ZMC_CUDA(cudaStreamIsCapturing(stream, &cs));
+        if (cs != cudaStreamCaptureStatusNone) return cuda_fail(cudaErrorStreamCaptureUnsupported);
+    }
 
     // ---- parameter block -----------------------------------------------------------------------
     ScanParams p;
@@ -550,7 +589,8 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     // ---- H1: the lists on the device (cached by content; a hit copies nothing) ----------------------------
     ListSlot* slot = nullptr;
     size_t h2d_bytes = 0;
-    st = stage_lists(s, M, lists, p.list_off, total, (o.flags & ZMC_OPT_FRESH_LISTS) != 0, stream, &slot, &h2d_bytes);
+    bool capturing = false;
+    st = stage_lists(s, M, lists, p.list_off, total, (o.flags & ZMC_OPT_FRESH_LISTS) != 0, stream, &slot, &h2d_bytes, &capturing);
     if (st != ZMC_OK) return st;
     p.lists = slot->dev;
     if (timing && h2d_bytes) { ZMC_CUDA(new_tev(&ev_h2d)); ZMC_CUDA(cudaEventRecord(ev_h2d, stream)); }
@@ -675,7 +715,7 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
             s->stage_used[buf] = true;
         }
     }
-    ZMC_CUDA(cudaEventRecord(slot->done, stream));
+    if (!capturing) ZMC_CUDA(cudaEventRecord(slot->done, stream));   // a captured slot is never evicted: nothing waits on `done`
     if (host_out) {   // join the side stream back into `stream`
         const int last = (int)((s->stage_rot - 1u) & 1u);
         ZMC_CUDA(cudaStreamWaitEvent(stream, s->stage_free[last], 0));

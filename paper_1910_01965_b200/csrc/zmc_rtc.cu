@@ -65,7 +65,7 @@ Nvrtc& nvrtc() {
 }
 
 std::mutex g_user_mutex;
-std::vector<std::unique_ptr<UserIntegrand>> g_users;
+std::vector<std::shared_ptr<UserIntegrand>> g_users;
 int g_next_user_id = kFirstUserId;        // ids are never reused
 thread_local std::string tl_compile_log;
 
@@ -134,17 +134,34 @@ template <typename R> struct FamUser {
 
 }  // namespace
 
-const UserIntegrand* find_user_integrand(int id) {
+std::shared_ptr<const UserIntegrand> find_user_integrand(int id) {
     std::lock_guard<std::mutex> lock(g_user_mutex);
     for (auto& u : g_users)
-        if (u->id == id) return u.get();
+        if (u->id == id) return u;
     return nullptr;
+}
+
+// Runs when the last holder lets go (the registry after the last unregister / zmc_shutdown, or a scan that was in progress
+// at that moment).  Kernels already enqueued may still be running: wait for every device that ever launched one before the
+// code is unloaded.
+UserIntegrand::~UserIntegrand() {
+    if (!lib) return;
+    const uint64_t mask = launched_on.load();
+    int cur = 0;
+    if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); return; }   // no runtime any more (process exit): nothing to unload
+    for (int d = 0; d < 64; ++d)
+        if (mask >> d & 1u) { if (cudaSetDevice(d) == cudaSuccess) cudaDeviceSynchronize(); }
+    cudaSetDevice(cur);
+    cudaLibraryUnload(lib);
+    cudaGetLastError();
 }
 
 cudaError_t launch_user(const UserIntegrand& u, int precision, int schedule, const ScanParams& p, void* out_mean,
                         void* out_stderr, int grid, size_t smem_bytes, cudaStream_t stream) {
     cudaKernel_t k = u.kern[precision][schedule - 1];
     if (!k) return cudaErrorInvalidDeviceFunction;
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) u.launched_on.fetch_or(1ull << dev);
     if (smem_bytes > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute((const void*)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return e;
@@ -155,9 +172,8 @@ cudaError_t launch_user(const UserIntegrand& u, int precision, int schedule, con
 
 void unload_user_integrands() {
     std::lock_guard<std::mutex> lock(g_user_mutex);
-    for (auto& u : g_users)
-        if (u->lib) cudaLibraryUnload(u->lib);
-    g_users.clear();                           // ids are valid until zmc_shutdown (include/zmc.h); they are never reused
+    g_users.clear();                           // ids are valid until zmc_shutdown (include/zmc.h); they are never reused.
+                                               // Each entry unloads its code when its last holder lets go (~UserIntegrand).
 }
 
 }  // namespace zmc
@@ -192,6 +208,7 @@ zmc_status zmc_register_integrand_ex(const char* name, const char* body, int N, 
         std::lock_guard<std::mutex> lock(g_user_mutex);
         for (auto& u : g_users)
             if (u->hash == h && u->lib && u->N == N && u->M == M && u->n_consts == n_consts && u->flags == flags && u->body == body) {
+                ++u->registrations;            // one more owner of this id: it takes as many unregister calls to drop it
                 *integrand_id = u->id;
                 return ZMC_OK;
             }
@@ -236,7 +253,7 @@ zmc_status zmc_register_integrand_ex(const char* name, const char* body, int N, 
     std::vector<char> cubin(cubin_size);
     if (rt.getCUBIN(prog, cubin.data()) != NVRTC_SUCCESS) return ZMC_ERR_COMPILE;
 
-    auto u = std::make_unique<UserIntegrand>();
+    auto u = std::make_shared<UserIntegrand>();
     u->name = name; u->N = N; u->M = M; u->n_consts = n_consts; u->flags = flags; u->body = body; u->hash = h;
     cudaError_t e = cudaLibraryLoadData(&u->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
     if (e != cudaSuccess) { tl_compile_log += "\ncudaLibraryLoadData: "; tl_compile_log += cudaGetErrorString(e); return ZMC_ERR_CUDA; }
@@ -245,10 +262,7 @@ zmc_status zmc_register_integrand_ex(const char* name, const char* body, int N, 
             const char* lowered = nullptr;
             const bool named = rt.getLoweredName(prog, expr[pr][sc].c_str(), &lowered) == NVRTC_SUCCESS && lowered;
             e = named ? cudaLibraryGetKernel(&u->kern[pr][sc], u->lib, lowered) : cudaErrorInvalidDeviceFunction;
-            if (e != cudaSuccess) {          // the loaded code is released on every failure after the load
-                cudaLibraryUnload(u->lib);
-                return named ? ZMC_ERR_CUDA : ZMC_ERR_COMPILE;
-            }
+            if (e != cudaSuccess) return named ? ZMC_ERR_CUDA : ZMC_ERR_COMPILE;   // ~UserIntegrand releases the loaded code
         }
     std::lock_guard<std::mutex> lock(g_user_mutex);
     u->id = g_next_user_id++;
@@ -265,9 +279,10 @@ zmc_status zmc_unregister_integrand(int integrand_id) {
     std::lock_guard<std::mutex> lock(g_user_mutex);
     for (size_t i = 0; i < g_users.size(); ++i)
         if (g_users[i]->id == integrand_id) {
-            if (g_users[i]->lib) cudaLibraryUnload(g_users[i]->lib);
+            if (--g_users[i]->registrations > 0) return ZMC_OK;      // registered more than once: other owners keep the id
+            std::shared_ptr<UserIntegrand> last = std::move(g_users[i]);
             g_users.erase(g_users.begin() + (long)i);
-            return ZMC_OK;
+            return ZMC_OK;                     // `last` goes out of scope here: unloads now unless a scan still holds the entry
         }
     return ZMC_ERR_UNKNOWN_INTEGRAND;
 }

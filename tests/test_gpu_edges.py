@@ -263,6 +263,52 @@ def test_a_scan_with_device_outputs_can_be_captured_into_a_cuda_graph():
         m2, e2, _ = zb.scan_workload(w2)
     torch.cuda.synchronize()
     assert bool(torch.isfinite(m2).all())
+    # The graph's kernel node holds the address of the library's cached copy of the lists.  That copy must have survived the
+    # ten other list sets above (every ordinary slot was recycled) -- and a much longer set, which makes slots reallocate.
+    big = wl.config(2, scale=[3000, 7], n_samples=16)
+    zb.scan_workload(big, count=64)
+    for k in range(9):
+        w3 = wl.config(2, scale=[3000 + k, 5], n_samples=16)
+        zb.scan_workload(w3, count=64)
+    torch.cuda.synchronize()
+    for _ in range(2):
+        m.zero_(); e.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(m, ref_m) and torch.equal(e, ref_e)
+
+
+def test_calls_that_cannot_be_captured_are_refused_during_capture():
+    """During stream capture a scan whose lists are not cached yet (it would have to upload), or one that asks for timing
+    (it would synchronise), returns ZMC_ERR_CUDA / cudaErrorStreamCaptureUnsupported and leaves the capture intact."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(1, scale=[19], n_samples=64)
+    w.lists[0] = wl.linspace(0.25, 7.75, 19)          # lists no other test uses: not in the cache
+    m = torch.zeros(w.G, dtype=torch.float64, device="cuda")
+    e = torch.zeros_like(m)
+    plan = zb.ScanPlan(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, m, e, precision=w.precision, consts=w.consts)
+    other = wl.config(1, scale=[23], n_samples=64)
+    m2 = torch.zeros(other.G, dtype=torch.float64, device="cuda")
+    e2 = torch.zeros_like(m2)
+    plan2 = zb.ScanPlan(other.integrand_id, other.bounds, other.lists, other.n_samples, other.seed, m2, e2)
+    s = torch.cuda.Stream()
+    plan2(s)                                          # `other` is cached, `w` is not
+    s.synchronize()
+    ref2 = m2.clone()
+    g = torch.cuda.CUDAGraph()
+    statuses = []
+    with torch.cuda.graph(g, stream=s):
+        for call, kw in ((plan, {}), (plan2, {"timing": True})):
+            with pytest.raises(zb.ZmcError) as exc:
+                call(torch.cuda.current_stream(), **kw)
+            statuses.append((exc.value.status, zb.load().zmc_last_cuda_error()))
+        plan2(torch.cuda.current_stream())            # the capture is still usable
+    assert statuses == [(zb.ZMC_ERR_CUDA, 900), (zb.ZMC_ERR_CUDA, 900)]
+    m2.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(m2, ref2) and not bool(m.any())
 
 
 def test_decode_of_a_full_2_pow_30_point_launch_with_awkward_list_lengths():

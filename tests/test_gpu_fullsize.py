@@ -12,6 +12,7 @@ import pytest
 from oracle import zmc_oracle as orc
 from paper_1910_01965_b200 import workloads as wl
 import closed_forms as cf
+from test_gpu_parity import assert_parity
 
 pytestmark = pytest.mark.gpu
 NT = min(16, os.cpu_count() or 1)
@@ -33,14 +34,7 @@ def check(w, mean, err, idx):
     assert rc == 0
     m = np.asarray(mean)[idx.astype(np.int64)].astype(np.float64)      # index first: `mean` may hold 10^10 elements
     e = np.asarray(err)[idx.astype(np.int64)].astype(np.float64)
-    if w.precision == wl.PREC_F64:
-        bad_m = np.abs(m - mean_o) > 1e-10 * np.maximum(np.abs(mean_o), err_o)
-        bad_e = np.abs(e - err_o) > 1e-10 * err_o
-    else:
-        bad_m = np.abs(m - mean_o) > 1e-4 * np.abs(mean_o) + 1e-6
-        bad_e = np.abs(e - err_o) > 1e-4 * np.abs(err_o) + 1e-6
-    assert not bad_m.any(), f"mean: {bad_m.sum()} of {len(idx)} sampled points off"
-    assert not bad_e.any(), f"stderr: {bad_e.sum()} of {len(idx)} sampled points off"
+    assert_parity(w, m, e, mean_o, err_o)          # the one tolerance rule of test_gpu_parity.py; records the margin
     return mean_o, err_o
 
 

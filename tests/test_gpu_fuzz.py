@@ -58,6 +58,4 @@ def test_random_configuration_matches_oracle(case):
     for g in (gm, ge):
         assert bool(torch.isnan(g[:pad]).all()) and bool(torch.isnan(g[pad + count:]).all()), "write outside the output range"
         assert not bool(torch.isnan(g[pad:pad + count]).any()), "an element of the range was not written"
-    b = np.asarray(w.bounds).reshape(-1, 2)
-    volume = float(np.prod(b[:, 1] - b[:, 0]))
-    assert_parity(w, m.cpu().numpy(), e.cpu().numpy(), mean_o, err_o, abs_scale=max(1.0, volume / 8.0))
+    assert_parity(w, m.cpu().numpy(), e.cpu().numpy(), mean_o, err_o)      # one tolerance rule, from the box (test_gpu_parity.py)

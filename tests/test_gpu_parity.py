@@ -2,9 +2,12 @@
 
 Tolerances (BASELINE.json north_star, reading Q12 in DESIGN.md):
   fp64 path : |d mean| <= 1e-10 * max(|mean_o|, stderr_o),  |d stderr| <= 1e-10 * stderr_o
-  F32E path : |d| <= 1e-4 * |oracle| + 1e-6   (mean and stderr) on the BASELINE configs (V <= 8);
-              for the paper's Eq. (2) boxes ([0,10]^N, V up to 1e4, phases up to 80 rad) the absolute
-              term scales with the volume: 1e-6 * V (fp32 evaluation error of g times V).
+  F32E path : |d| <= 1e-4 * |oracle| + 1e-6 * max(1, V / 8)   (mean and stderr): north_star's tolerance as
+              written on the BASELINE configs (V <= 8); on larger boxes (the paper's Eq. (2) [0,10]^N, the fuzz
+              test's random boxes) the absolute term grows with the volume, normalised to cfg 5's V = 8 -- ONE
+              rule, applied by assert_parity from the workload's own box.
+Every assert_parity call also records its worst |d| / tolerance; conftest.py prints them at the end of the run
+("parity margins"), so the log shows the margin and not only pass / fail.
 """
 import os
 
@@ -25,20 +28,28 @@ def _zb():
     return binding
 
 
-def assert_parity(w, mean, err, mean_o, err_o, abs_scale=1.0, eps_g=0.0):
+MARGINS = []      # (test id, worst |d mean| / tol, worst |d stderr| / tol, points) -- printed by conftest.py
+
+
+def assert_parity(w, mean, err, mean_o, err_o, eps_g=0.0):
     """eps_g: the per-sample disagreement |g_gpu - g_oracle| the two evaluations of g may have (DESIGN.md section 2,
     "nearly constant integrands"): it moves the stderr by at most V eps_g / sqrt(n-1) whatever the spread of g is."""
     mean, err = np.asarray(mean, dtype=np.float64), np.asarray(err, dtype=np.float64)
+    b = np.asarray(w.bounds).reshape(-1, 2)
+    volume = float(np.prod(b[:, 1] - b[:, 0]))
     if w.precision == wl.PREC_F64 and not w.out_f32:
-        b = np.asarray(w.bounds).reshape(-1, 2)
-        floor = float(np.prod(b[:, 1] - b[:, 0])) * eps_g / np.sqrt(w.n_samples - 1.0)
-        tol_m = 1e-10 * np.maximum(np.abs(mean_o), err_o)
-        tol_e = 1e-10 * err_o + floor
-        bad_m = np.abs(mean - mean_o) > tol_m + 1e-300
-        bad_e = np.abs(err - err_o) > tol_e + 1e-300
+        floor = volume * eps_g / np.sqrt(w.n_samples - 1.0)
+        tol_m = 1e-10 * np.maximum(np.abs(mean_o), err_o) + 1e-300
+        tol_e = 1e-10 * err_o + floor + 1e-300
     else:
-        bad_m = np.abs(mean - mean_o) > 1e-4 * np.abs(mean_o) + 1e-6 * abs_scale
-        bad_e = np.abs(err - err_o) > 1e-4 * np.abs(err_o) + 1e-6 * abs_scale
+        abs_term = 1e-6 * max(1.0, volume / 8.0)
+        tol_m = 1e-4 * np.abs(mean_o) + abs_term
+        tol_e = 1e-4 * np.abs(err_o) + abs_term
+    ratio_m, ratio_e = np.abs(mean - mean_o) / tol_m, np.abs(err - err_o) / tol_e
+    if len(mean):
+        test_id = os.environ.get("PYTEST_CURRENT_TEST", "?").split(" ")[0].split("::", 1)[-1]
+        MARGINS.append((test_id, float(np.nanmax(ratio_m)), float(np.nanmax(ratio_e)), len(mean)))
+    bad_m, bad_e = ~(ratio_m <= 1.0), ~(ratio_e <= 1.0)         # a NaN anywhere is a failure
     assert not bad_m.any(), f"mean: {bad_m.sum()} of {len(mean)} off, worst {np.abs(mean - mean_o).max()}"
     assert not bad_e.any(), f"stderr: {bad_e.sum()} of {len(err)} off, worst {np.abs(err - err_o).max()}"
 
@@ -64,7 +75,19 @@ REDUCED = {
     "eq2_M4_N4_f32": lambda: wl.paper_eq2(4, 4, n_samples=500, L=7, precision=wl.PREC_F32E),
     "eq4": lambda: wl.paper_eq4(n_samples=3000, L=6),
     "eq4_f32": lambda: wl.paper_eq4(n_samples=3000, L=6, precision=wl.PREC_F32E),
+    # reading S5 on a box whose bounds, widths and constant are not exactly representable in float (the oracle's side of
+    # these roundings is pinned by the S5_BOX cases of test_oracle_pins.py)
+    "s5_box_c3_f64": lambda: _c3_s5_box(wl.PREC_F64),
+    "s5_box_c3_f32": lambda: _c3_s5_box(wl.PREC_F32E),
 }
+
+
+def _c3_s5_box(precision):
+    w = wl.config(3, scale=[7, 5, 6], n_samples=1501)
+    w.bounds = np.array([0.1, 0.7, -0.3, 1.9, 0.2, 1.3])
+    w.consts = np.array([0.6])
+    w.precision = precision
+    return w
 
 
 def _c3_n(N):
@@ -81,9 +104,7 @@ def test_parity_reduced(name, sched):
     rc, mean_o, err_o = orc.scan_workload(w, n_threads=NT)
     assert rc == 0
     mean, err = run_gpu(w, schedule=SCHEDS[sched])
-    b = np.asarray(w.bounds).reshape(-1, 2)
-    volume = float(np.prod(b[:, 1] - b[:, 0]))
-    assert_parity(w, mean, err, mean_o, err_o, abs_scale=volume if name.startswith("eq2") else 1.0)
+    assert_parity(w, mean, err, mean_o, err_o)
 
 
 @pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5", "eq4_f32"])

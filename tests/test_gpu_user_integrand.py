@@ -115,7 +115,9 @@ def test_registration_is_cached_by_content_and_can_be_undone():
     zb.zmc_scan_ex(uid, [0.0, 1.0], [np.array([1.0, 2.0, 3.0])], 64, 1, m, e)
     torch.cuda.synchronize()
     assert torch.all(m > 0.125)
-    zb.zmc_unregister_integrand(uid)
+    zb.zmc_unregister_integrand(uid)                     # registered twice above: registrations are counted ...
+    zb.zmc_scan_ex(uid, [0.0, 1.0], [np.array([1.0, 2.0, 3.0])], 64, 1, m, e)
+    zb.zmc_unregister_integrand(uid)                     # ... and the second unregister drops the id
     with pytest.raises(zb.ZmcError) as ei:
         zb.zmc_scan_ex(uid, [0.0, 1.0], [np.array([1.0, 2.0, 3.0])], 64, 1, m, e)
     assert ei.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
@@ -124,3 +126,45 @@ def test_registration_is_cached_by_content_and_can_be_undone():
     assert ei.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
     fresh = zb.zmc_register_integrand("cached", body, 1, 1, 0)          # compiled again, ids are never reused
     assert fresh != uid
+
+
+def test_an_id_registered_twice_survives_the_first_unregister():
+    """Two parts of a program register the same body and get the same id; one of them unregistering must not pull the
+    code from under the other (include/zmc.h, zmc_unregister_integrand: registrations are counted)."""
+    from paper_1910_01965_b200 import binding as zb
+    body = "return exp(-x[0] * y[0]) + c[0] * y[1];"
+    first = zb.zmc_register_integrand("owner_a", body, 2, 1, 1)
+    second = zb.zmc_register_integrand("owner_b", body, 2, 1, 1)
+    assert first == second
+    w = wl.Workload("shared", first, np.array([0.0, 1.0, 0.0, 2.0]), [wl.linspace(0.1, 2.0, 17)], 301, 4, wl.PREC_F64,
+                    np.array([0.75]))
+    before, before_err = run_gpu(w, schedule=2)
+    zb.zmc_unregister_integrand(first)                 # owner_a is done with it
+    after, after_err = run_gpu(w, schedule=2)          # owner_b still scans
+    assert np.array_equal(before, after) and np.array_equal(before_err, after_err)
+    zb.zmc_unregister_integrand(second)
+    with pytest.raises(zb.ZmcError) as exc:
+        run_gpu(w, schedule=2)
+    assert exc.value.status == zb.ZMC_ERR_UNKNOWN_INTEGRAND
+    with pytest.raises(zb.ZmcError):
+        zb.zmc_unregister_integrand(second)
+
+
+def test_unregister_right_after_an_enqueue_only_scan():
+    """zmc_scan_ex only enqueues; unregistering the integrand before the kernels have run must wait for them instead of
+    unloading code that is still executing."""
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    body = "R s = x[0]; for (int k = 0; k < 3; ++k) s += y[k] * x[1]; return cos(s);"
+    w = wl.Workload("inflight", 0, np.array([0.0, 1.0] * 3), [wl.linspace(0.1, 2.0, 400), wl.linspace(0.5, 1.5, 300)],
+                    4000, 8, wl.PREC_F64, np.zeros(0))
+    w.integrand_id = zb.zmc_register_integrand("inflight", body, 3, 2, 0)
+    ref, ref_err = run_gpu(w, schedule=1)
+    mean = torch.zeros(w.G, dtype=torch.float64, device="cuda")
+    err = torch.zeros_like(mean)
+    zb.zmc_scan_ex(w.integrand_id, w.bounds, w.lists, w.n_samples, w.seed, mean, err, schedule=1)    # ~10 ms of GPU work, not waited for
+    zb.zmc_unregister_integrand(w.integrand_id)
+    torch.cuda.synchronize()
+    assert np.array_equal(mean.cpu().numpy(), ref) and np.array_equal(err.cpu().numpy(), ref_err)
+    with pytest.raises(zb.ZmcError):
+        run_gpu(w, schedule=1)
