@@ -8,8 +8,10 @@ store) over one synthetic workload of BASELINE.json `configs`.  The default work
 single-GPU configuration (10^10 grid points x 256 samples): `value` is integrand
 evaluations/s with the 80 GB of results device-resident, `e2e` the same scan through the C ABI with pinned HOST
 outputs (list H2D forced, result D2H streamed in 2^28-point batches, `exposed_d2h_ms` = what compute did not hide).
-`per_config` carries the same record for cfg1-cfg4 (the north_star target is on cfg2-cfg4), `pipe_rates` the
-dispatch costs measured in this very run (zmc_measure_pipes) that the ALU roofline is built from, `cpu_baseline`
+`per_config_detail` carries the same record for cfg1-cfg4 (the north_star target is on cfg2-cfg4) and `per_config`, near
+the end of the line, their headline numbers; `roofline.frac` is the builder's dispatch model, `roofline.frac_survey`
+SURVEY.md 8(d)'s own instruction table; `pipe_rates` the
+dispatch costs measured in this very run (bench_probe.py, its own libzmc_probe.so) that the ALU roofline is built from, `cpu_baseline`
 the unoptimised CPU oracle on a bounded slice.  With N > 1 (torchrun) the grid's first list is lengthened N-fold and
 each rank scans its own contiguous flat range -- no data-path collective.
 """
@@ -66,6 +68,13 @@ PER_CONFIG = ["cfg1", "cfg2", "cfg3", "cfg4"]
 # `ncu --set full` capture of each kernel (profiles/r02_kernel.md).  cfg5: per 2^28-point batch launch (algorithmic:
 # 2^28 x 8 B = 2.147e9 written); cfg4: 1e8 x 16 B = 1.6e9; cfg2: its 16 MB of results never leave L2 during the kernel.
 NCU_TRAFFIC_BYTES = {"cfg5": 28.094464e6 + 2.096151e9, "cfg4": 37.298176e6 + 1.556428e9, "cfg2": 40.96e3 + 0.0}
+NCU_TRAFFIC_SOURCE = "stored constant: one `ncu --set full` capture of this kernel (profiles/r02_kernel.md), NOT measured in this run"
+# SURVEY.md 8(d) as written: I_min thread-instructions per evaluation and the IMAD.WIDE count per evaluation of its table
+# (Philox with all 20 IMAD.WIDE per block), for `roofline.frac_survey` = max(I_min, 4 n_IMAD.WIDE) lane-cycles per evaluation:
+# the issue bound (128 thread-instructions per clock per SM) or, by the survey's own sensitivity clause, the FMA-heavy pipe at
+# 32 IMAD.WIDE per clock per SM (= 4 lane-cycles each; ncu shows 3.3-3.9 FMA-heavy cycles per instruction, profiles/r02_kernel.md section 3).
+SURVEY_I_MIN = {"cfg1": (45.0, 5), "cfg2": (57.0, 10), "cfg3": (54.0, 20), "cfg4": (84.5, 30), "cfg5": (53.0, 15)}
+IMAD_WIDE_LANE_CYCLES = 4.0
 
 
 def w_min(name):
@@ -410,6 +419,8 @@ def main():
         w_cyc, w_bound, w_res, w_add = w_min(w.name)
         rate = evals_rank / (kernel_ms * 1e-3)
         achieved = w_cyc * rate / 1e9
+        sv = SURVEY_I_MIN.get(USER_BODIES[w.name][0] if w.name in USER_BODIES else w.name)
+        sv_cyc = max(sv[0], IMAD_WIDE_LANE_CYCLES * sv[1]) if sv else None
         return {
             "config": cfg, "w": w,
             "value": evals_all / (ms_per_step * 1e-3), "points_per_s": G_scan / (ms_per_step * 1e-3),
@@ -419,11 +430,20 @@ def main():
             "adaptive": adaptive, "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
                          "frac": achieved / PEAK_GLANE, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+                         "traffic_source": NCU_TRAFFIC_SOURCE if w.name in NCU_TRAFFIC_BYTES else None,
+                         # the same rate against SURVEY.md 8(d)'s own instruction table (see SURVEY_I_MIN above)
+                         "frac_survey": sv_cyc * rate / 1e9 / PEAK_GLANE if sv else None,
+                         "survey_lane_cycles_per_eval": sv_cyc,
+                         "survey_binding": (None if not sv else "issue (I_min)" if sv[0] >= IMAD_WIDE_LANE_CYCLES * sv[1]
+                                            else "FMA-heavy pipe (4 lane-cycles per IMAD.WIDE)"),
                          "lane_cycles_per_eval": w_cyc, "binding_resource": w_bound, "resources": w_res,
                          "measured_lane_cycles_per_eval": PEAK_GLANE * 1e9 * (clocks["sm_mhz"] or SM_MAX_MHZ) / SM_MAX_MHZ / rate,
                          "lane_cycles_per_eval_no_overlap": w_add, "frac_no_overlap": w_add * rate / 1e9 / PEAK_GLANE,
-                         "peak_source": "148 SMs x 4 SMSPs x 32 lanes x 1965 MHz dispatch; per-class costs: pipe_rates in this "
-                                        "line (zmc_measure_pipes), DESIGN.md section 6",
+                         "peak_source": "peak = 148 SMs x 4 SMSPs x 32 lanes x 1965 MHz dispatch slots (sm_max_mhz of MEASURED_PEAKS.json; "
+                                        "its HBM / bf16 figures do not apply: ALU-bound, no contraction). `frac` counts the builder's W_min "
+                                        "(serial-dispatch model: integer 2, FP32 1 lane-cycles on one port; per-class costs re-measured in "
+                                        "this run, pipe_rates; DESIGN.md section 6). `frac_survey` counts SURVEY.md 8(d)'s table: "
+                                        "max(I_min, 4 x IMAD.WIDE) lane-cycles per evaluation",
                          "frac_at_measured_clock": (achieved / (PEAK_GLANE * clocks["sm_mhz"] / SM_MAX_MHZ)
                                                     if clocks.get("sm_mhz") else None)},
         }
@@ -440,9 +460,10 @@ def main():
             per_config[name]["n_samples"] = r["config"]["n_samples"]
     pipes = None
     if not args.no_pipe_rates and rank == 0:
-        rep = zb.zmc_measure_pipes(stream)
-        pipes = {"sm_mhz": rep["sm_mhz"], "unit": "SMSP-cycles per group per warp: [measured, if independent pipes, if one shared pipe]",
-                 "rows": {r["name"]: [round(r["cycles"], 3), round(r["parallel"], 3), round(r["serial"], 3)] for r in rep["rows"]}}
+        import bench_probe                       # a tool beside bench.py with its own libzmc_probe.so: not part of libzmc.so
+        rep = bench_probe.measure_pipes(stream.cuda_stream)
+        pipes = {"sm_mhz": round(rep["sm_mhz"], 1), "unit": "SMSP-cycles per group per warp: [measured, if independent pipes, if one shared pipe]",
+                 "rows": {r["name"]: [round(r["cycles"], 2), round(r["parallel"], 2), round(r["serial"], 2)] for r in rep["rows"]}}
 
     if rank != 0:
         if world > 1:
@@ -451,7 +472,10 @@ def main():
 
     w = main_rec.pop("w")
     launches = main_rec["gpu_launches"] + sum(p["gpu_launches"] for p in per_config.values())
+    # Key order: the bulky records first, the contract keys after them, and a compact per-config table plus the CPU baseline
+    # last -- whoever keeps only the tail of this line still sees every headline number.
     out = {
+        "pipe_rates": pipes, "per_config_detail": per_config or None,
         "metric": METRIC, "value": main_rec["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": main_rec["ms_per_step"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": (main_rec["value"] / PUBLISHED_EVALS_PER_S[w.name] if w.name in PUBLISHED_EVALS_PER_S and world == 1 else None),
@@ -460,8 +484,13 @@ def main():
         "points_per_s": main_rec["points_per_s"], "kernel_ms_per_step": main_rec["kernel_ms_per_step"],
         "schedule_used": main_rec["schedule_used"], "clocks": main_rec["clocks"], "e2e": main_rec["e2e"],
         "farm": main_rec["farm"], "adaptive": main_rec["adaptive"], "gpu_launches": launches,
-        "roofline": main_rec["roofline"], "per_config": per_config or None, "pipe_rates": pipes,
+        "roofline": main_rec["roofline"],
     }
+    if per_config:
+        out["per_config"] = {"columns": ["evals_per_s", "kernel_ms", "roofline_frac", "roofline_frac_survey", "e2e_evals_per_s"],
+                             **{k: [float("%.4g" % v["value"]), round(v["kernel_ms_per_step"], 4), round(v["roofline"]["frac"], 3),
+                                    round(v["roofline"]["frac_survey"], 3), float("%.4g" % v["e2e"]["value"]) if v["e2e"] else None]
+                                for k, v in per_config.items()}}
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(w)
     print(json.dumps(out))

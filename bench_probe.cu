@@ -1,5 +1,7 @@
-// zmc_probe.cu -- zmc_measure_pipes(): the roofline denominators of the zmc_scan hot loop, measured on the device the
+// bench_probe.cu -- bench_measure_pipes(): the roofline denominators of the zmc_scan hot loop, measured on the device the
 // call runs on ("re-measure by micro-benchmark, these are the denominators").
+// A MEASUREMENT TOOL of bench.py, not part of the product: built into its own libzmc_probe.so (bench_probe.py), declared in
+// bench_probe.h; libzmc.so and include/zmc.h hold only the method's calls.  It shares no code with the library.
 //
 // The loop is ALU work -- a scalar integer hash (Philox: IMAD.WIDE + LOP3), a few FMAs and one transcendental per
 // sample -- so its ceiling is how many warp-instructions of each class an SM sub-partition (SMSP) can dispatch per
@@ -16,8 +18,10 @@
 #include <cstdio>
 #include <cstring>
 
-#include "zmc_internal.h"
-#include "zmc_params.h"
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "bench_probe.h"
 
 namespace {
 
@@ -234,7 +238,7 @@ struct Probe {
     double mhz;
     cudaEvent_t a, b;
     cudaError_t err = cudaSuccess;
-    zmc_pipe_report* rep;
+    bench_pipe_report* rep;
 
     template <class K, class... Args> double time_ms(K kern, Args... args) {
         float best = 1e30f;
@@ -255,8 +259,8 @@ struct Probe {
         return ms * 1e-3 * mhz * 1e6 / (groups_per_warp * warps_per_smsp);
     }
     void add(const char* name, double cyc, double parallel, double serial) {
-        if (rep->n_rows >= ZMC_PIPE_MAX_ROWS) return;
-        zmc_pipe_row& row = rep->rows[rep->n_rows++];
+        if (rep->n_rows >= BENCH_PIPE_MAX_ROWS) return;
+        bench_pipe_row& row = rep->rows[rep->n_rows++];
         std::snprintf(row.name, sizeof(row.name), "%s", name);
         row.cycles = cyc; row.parallel = parallel; row.serial = serial;
     }
@@ -280,19 +284,19 @@ struct Probe {
 
 }  // namespace
 
-extern "C" zmc_status zmc_measure_pipes(zmc_pipe_report* report, void* stream_v) {
-    if (!report) return ZMC_ERR_INVALID_ARG;
+extern "C" __attribute__((visibility("default"))) int bench_measure_pipes(bench_pipe_report* report, void* stream_v) {
+    if (!report) return -1;
     std::memset(report, 0, sizeof(*report));
     Probe p;
     p.rep = report;
     p.stream = static_cast<cudaStream_t>(stream_v);
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-        return ZMC_ERR_CUDA;
+        return (int)cudaGetLastError();
     p.grid = sms * 4;
     long long* clk = nullptr;
-    if (cudaMalloc(&p.out, (size_t)p.grid * 256 * sizeof(uint32_t)) != cudaSuccess) return ZMC_ERR_OUT_OF_MEMORY;
-    if (cudaMalloc(&clk, 2 * sizeof(long long)) != cudaSuccess) { cudaFree(p.out); return ZMC_ERR_OUT_OF_MEMORY; }
+    if (cudaMalloc(&p.out, (size_t)p.grid * 256 * sizeof(uint32_t)) != cudaSuccess) return (int)cudaErrorMemoryAllocation;
+    if (cudaMalloc(&clk, 2 * sizeof(long long)) != cudaSuccess) { cudaFree(p.out); return (int)cudaErrorMemoryAllocation; }
     cudaEventCreate(&p.a);
     cudaEventCreate(&p.b);
     p.mhz = 1.0;
@@ -354,6 +358,5 @@ extern "C" zmc_status zmc_measure_pipes(zmc_pipe_report* report, void* stream_v)
     cudaEventDestroy(p.b);
     cudaFree(p.out);
     cudaFree(clk);
-    if (p.err != cudaSuccess) { zmc::set_last_cuda_error((int)p.err); return ZMC_ERR_CUDA; }
-    return ZMC_OK;
+    return (int)p.err;                     // 0 = cudaSuccess, else the first cudaError_t met
 }

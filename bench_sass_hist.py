@@ -1,7 +1,10 @@
 """Hot-loop SASS histogram of the built kernels, per integrand evaluation, beside the algorithmic instruction list the
 ALU roofline is built from (bench.py ALG_OPS).
 
-    python -m paper_1910_01965_b200.sass_hist            # needs only the built objects (nvcc/cuobjdump, no GPU)
+    python bench_sass_hist.py            # needs only the built objects (nvcc/cuobjdump, no GPU)
+
+A measurement tool kept beside bench.py, outside the product package, so that profiles/r0N_sass_hist.txt stays
+reproducible from a committed command.
 
 For each BASELINE config the kernel bench.py actually launches (AUTO schedule) is disassembled with `cuobjdump -sass`,
 its innermost-longest loop (the sample loop) is located by its backward branch, and the opcodes in it are counted and
@@ -17,7 +20,7 @@ import re
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-OBJ = os.path.join(HERE, os.environ.get("ZMC_OBJ", "build"))
+OBJ = os.path.join(HERE, "paper_1910_01965_b200", os.environ.get("ZMC_OBJ", "build"))
 
 # config -> (object, substrings of the demangled kernel name, evaluations per loop trip, ALG_OPS (int, fp32, fp64, xu))
 KERNELS = {

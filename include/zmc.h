@@ -145,21 +145,6 @@ typedef struct zmc_farm_timing {
     double busy_ms[ZMC_MAX_FARM_DEVICES];            /* first pull to last completion, per device slot */
 } zmc_farm_timing;
 
-/* zmc_measure_pipes: one measured row.  All three numbers are SM-sub-partition cycles per group of instructions per warp. */
-#define ZMC_PIPE_MAX_ROWS 48
-typedef struct zmc_pipe_row {
-    char name[72];           /* e.g. "LOP3", "1xIMAD.WIDE+LOP3 + 2xDFMA, same warp", "cfg2 block: both, same warp (ptxas order)" */
-    double cycles;           /* measured */
-    double parallel;         /* max of the parts' own costs: what independent pipes would give */
-    double serial;           /* sum of the parts' own costs: what one shared pipe would give */
-} zmc_pipe_row;
-typedef struct zmc_pipe_report {
-    double sm_mhz;           /* SM clock while measuring (clock64 against globaltimer) */
-    int32_t sm_count;
-    int32_t n_rows;
-    zmc_pipe_row rows[ZMC_PIPE_MAX_ROWS];
-} zmc_pipe_report;
-
 typedef struct zmc_integrand_info {
     int32_t id;
     const char* name;
@@ -317,15 +302,6 @@ ZMC_API zmc_status zmc_register_integrand_ex(const char* name, const char* body,
  * loaded until it returns.  ZMC_ERR_UNKNOWN_INTEGRAND if the id is not (or no longer) registered. */
 ZMC_API zmc_status zmc_unregister_integrand(int integrand_id);
 ZMC_API const char* zmc_last_compile_log(void);   /* NVRTC log of the last zmc_register_integrand on this thread */
-/*
- * zmc_measure_pipes -- the roofline denominators of the hot loop, measured on the current device (the
- * loop is bound by ALU dispatch, "re-measure by micro-benchmark, these are the denominators").  Runs ~35 short synthetic
- * kernels (about 0.1 s) on `stream` and synchronises: the dispatch cost of every instruction class the loop uses, which
- * pairs of classes overlap (in one warp, and across warps), and cfg 2's instruction mix per Philox block.
- * section 6 explains how the ALU roofline is built from these rows; bench.py embeds them in its JSON line.
- */
-ZMC_API zmc_status zmc_measure_pipes(zmc_pipe_report* report, void* stream);
-
 /* Free the cached per-device scratch (staging buffers, streams, events) and unload user integrands. */
 ZMC_API void zmc_shutdown(void);
 #endif /* !__CUDACC_RTC__ */

@@ -35,7 +35,7 @@ EXPORTS = ["zmc_scan", "zmc_scan_ex", "zmc_integrand_count", "zmc_integrand_info
            "zmc_validate", "zmc_pick_schedule", "zmc_batch_range", "zmc_shutdown",
            "zmc_register_integrand", "zmc_last_compile_log", "zmc_scan_farm", "zmc_scan_adaptive",
            "zmc_pick_schedule_ex", "zmc_register_integrand_ex", "zmc_unregister_integrand", "zmc_scan_farm_adaptive",
-           "zmc_measure_pipes", "zmc_scan_noalloc"]
+           "zmc_scan_noalloc"]
 
 
 class zmc_param_list(ctypes.Structure):
@@ -67,19 +67,6 @@ class zmc_farm_timing(ctypes.Structure):
     _fields_ = [("wall_ms", ctypes.c_double), ("n_batches", ctypes.c_int64), ("batch_points", ctypes.c_uint64),
                 ("n_devices", ctypes.c_int32), ("reserved", ctypes.c_int32),
                 ("batches_done", ctypes.c_int64 * ZMC_MAX_FARM_DEVICES), ("busy_ms", ctypes.c_double * ZMC_MAX_FARM_DEVICES)]
-
-
-ZMC_PIPE_MAX_ROWS = 48
-
-
-class zmc_pipe_row(ctypes.Structure):
-    _fields_ = [("name", ctypes.c_char * 72), ("cycles", ctypes.c_double), ("parallel", ctypes.c_double),
-                ("serial", ctypes.c_double)]
-
-
-class zmc_pipe_report(ctypes.Structure):
-    _fields_ = [("sm_mhz", ctypes.c_double), ("sm_count", ctypes.c_int32), ("n_rows", ctypes.c_int32),
-                ("rows", zmc_pipe_row * ZMC_PIPE_MAX_ROWS)]
 
 
 class zmc_integrand_info(ctypes.Structure):
@@ -151,8 +138,6 @@ def load():
     lib.zmc_register_integrand_ex.restype = ctypes.c_int
     lib.zmc_unregister_integrand.argtypes = [ctypes.c_int]
     lib.zmc_unregister_integrand.restype = ctypes.c_int
-    lib.zmc_measure_pipes.argtypes = [P(zmc_pipe_report), ctypes.c_void_p]
-    lib.zmc_measure_pipes.restype = ctypes.c_int
     lib.zmc_scan_farm.argtypes = scan_args[:9] + [P(ctypes.c_int), ctypes.c_int, P(zmc_options), P(zmc_farm_timing)]
     lib.zmc_scan_farm.restype = ctypes.c_int
     lib.zmc_scan_adaptive.argtypes = scan_args[:5] + [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_double, ctypes.c_uint64,
@@ -470,15 +455,6 @@ def zmc_scan_farm_adaptive(integrand_id: int, bounds, lists, n_first: int, n_max
     n = tm.n_devices
     return {"wall_ms": tm.wall_ms, "n_batches": tm.n_batches, "batch_points": tm.batch_points, "n_devices": n,
             "batches_done": list(tm.batches_done[:n]), "busy_ms": list(tm.busy_ms[:n])}
-
-
-def zmc_measure_pipes(stream=None) -> dict:
-    """include/zmc.h zmc_measure_pipes: the measured dispatch costs behind the ALU roofline."""
-    rep = zmc_pipe_report()
-    _check(load().zmc_measure_pipes(ctypes.byref(rep), ctypes.c_void_p(_stream_handle(stream))))
-    return {"sm_mhz": rep.sm_mhz, "sm_count": rep.sm_count,
-            "rows": [{"name": rep.rows[i].name.decode(), "cycles": rep.rows[i].cycles, "parallel": rep.rows[i].parallel,
-                      "serial": rep.rows[i].serial} for i in range(rep.n_rows)]}
 
 
 def zmc_unregister_integrand(integrand_id: int):

@@ -28,15 +28,17 @@ def test_struct_layouts_match_header_sizes(tmp_path):
     import ctypes
     import subprocess
     src = tmp_path / "sz.c"
-    src.write_text('#include <stdio.h>\n#include "zmc.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu\\n",'
+    # (bench_probe.h, the header of bench.py's separate micro-benchmark library, is checked the same way against bench_probe.py)
+    import bench_probe
+    src.write_text('#include <stdio.h>\n#include "zmc.h"\n#include "bench_probe.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu\\n",'
                    'sizeof(zmc_options),sizeof(zmc_timing),sizeof(zmc_param_list),sizeof(zmc_integrand_info),'
-                   'sizeof(zmc_pipe_report),sizeof(zmc_farm_timing));return 0;}\n')
+                   'sizeof(bench_pipe_report),sizeof(zmc_farm_timing));return 0;}\n')
     exe = tmp_path / "sz"
-    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)],
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-I", ROOT, str(src), "-o", str(exe)],
                    check=True)
     sizes = [int(v) for v in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
     assert sizes == [ctypes.sizeof(zb.zmc_options), ctypes.sizeof(zb.zmc_timing), ctypes.sizeof(zb.zmc_param_list),
-                     ctypes.sizeof(zb.zmc_integrand_info), ctypes.sizeof(zb.zmc_pipe_report), ctypes.sizeof(zb.zmc_farm_timing)]
+                     ctypes.sizeof(zb.zmc_integrand_info), ctypes.sizeof(bench_probe._Report), ctypes.sizeof(zb.zmc_farm_timing)]
 
 
 def test_integrand_table():

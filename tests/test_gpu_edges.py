@@ -126,11 +126,12 @@ def test_back_to_back_host_output_scans_on_two_streams_and_after_shutdown():
 
 
 def test_measure_pipes_reports_the_dispatch_costs_the_roofline_uses():
-    """zmc_measure_pipes (include/zmc.h): the rows bench.py prints as `pipe_rates`.  Sanity bands only -- the numbers are
+    """bench_probe.py (bench.py's micro-benchmark, its own libzmc_probe.so): the rows bench.py prints as `pipe_rates`.  Sanity bands only -- the numbers are
     measurements -- around what DESIGN.md section 6 builds the ALU roofline from: integer 2 cycles per warp-instruction,
     FP32 1, FP64 2, XU 8, and a `serial >= parallel` pair of bounds on every mixed row."""
-    from paper_1910_01965_b200 import binding as zb
-    rep = zb.zmc_measure_pipes()
+    import torch
+    import bench_probe
+    rep = bench_probe.measure_pipes(torch.cuda.current_stream().cuda_stream)
     rows = {r["name"]: r for r in rep["rows"]}
     assert rep["sm_count"] >= 1 and 500.0 < rep["sm_mhz"] < 3000.0 and len(rows) >= 40
     for name, lo, hi in [("LOP3", 1.8, 2.6), ("SHF", 1.8, 2.6), ("IMAD.WIDE+LOP3", 3.6, 5.0), ("FFMA", 0.9, 1.5),
