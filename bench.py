@@ -9,8 +9,8 @@ single-GPU configuration (10^10 grid points x 256 samples, SURVEY.md section 8 t
 evaluations/s with the 80 GB of results device-resident, `e2e` the same scan through the C ABI with pinned HOST
 outputs (list H2D forced, result D2H streamed in 2^28-point batches, `exposed_d2h_ms` = what compute did not hide).
 `per_config_detail` carries the same record for cfg1-cfg4 (the north_star target is on cfg2-cfg4) and `per_config`, near
-the end of the line, their headline numbers; `roofline.frac` is the builder's dispatch model, `roofline.frac_survey`
-SURVEY.md 8(d)'s own instruction table; `pipe_rates` the
+the end of the line, their headline numbers; `roofline.frac` is measured against the busiest physical unit (ncu-measured pipe occupancy per
+instruction class), `frac_dispatch_model` the round-2 dispatch model, `frac_survey` SURVEY.md 8(d)'s own table; `pipe_rates` the
 dispatch costs measured in this very run (bench_probe.py, its own libzmc_probe.so) that the ALU roofline is built from, `cpu_baseline`
 the unoptimised CPU oracle on a bounded slice.  With N > 1 (torchrun) the grid's first list is lengthened N-fold and
 each rank scans its own contiguous flat range -- no data-path collective.
@@ -84,6 +84,24 @@ def w_min(name):
     # what the same list costs if FP64 / XU instructions do NOT hide behind the integer stream but take one dispatch
     # cycle each (what zmc_measure_pipes' "same warp" rows and every kernel of this library show on sm_100)
     return res[bound], bound, res, 2 * i + f + d + xu
+
+
+# The PHYSICAL units, with the occupancy ncu reads for one warp-instruction of each class (profiles/r03_probe_ncu.md: each
+# single-class probe kernel drives its pipe to 97-99.8 % busy at exactly these rates): IMAD.WIDE / IMAD.HI hold the
+# FMA-heavy pipe 4 SMSP-cycles, FP32 instructions 1 cycle on FMA-heavy or FMA-lite (half each), LOP3 / SHF / IADD3 the ALU pipe
+# 2 cycles, FP64 its pipe 2 cycles, MUFU / F2F the XU 8 cycles; every instruction takes one issue slot.  16 of a hoisted
+# Philox block's 34 integer instructions are IMAD.WIDE.  Lane-cycles per evaluation on the busiest unit:
+PHILOX_BLOCKS = {"cfg1": 0.25, "cfg2": 0.5, "cfg3": 1.0, "cfg4": 1.5, "cfg5": 0.75, "eq4": 1.5}
+
+
+def pipe_bound(name):
+    base = USER_BODIES[name][0] if name in USER_BODIES else ("eq4" if name.startswith("eq4") else name)
+    i, f, d, xu = ALG_OPS[name]
+    wide = 16.0 * PHILOX_BLOCKS[base]
+    res = {"fma_heavy(4*IMAD.WIDE+fp32/2)": 4 * wide + f / 2, "alu(2*other int)": 2 * (i - wide), "fp64": 2 * d, "xu": 8 * xu,
+           "issue": i + f + d + xu}
+    bound = max(res, key=res.get)
+    return res[bound], bound, res
 
 
 SM_COUNT, LANES_PER_SM_CLK, SM_MAX_MHZ = 148, 128, 1965.0
@@ -419,6 +437,7 @@ def main():
         w_cyc, w_bound, w_res, w_add = w_min(w.name)
         rate = evals_rank / (kernel_ms * 1e-3)
         achieved = w_cyc * rate / 1e9
+        pb_cyc, pb_bound, pb_res = pipe_bound(w.name)
         sv = SURVEY_I_MIN.get(USER_BODIES[w.name][0] if w.name in USER_BODIES else w.name)
         sv_cyc = max(sv[0], IMAD_WIDE_LANE_CYCLES * sv[1]) if sv else None
         return {
@@ -428,8 +447,12 @@ def main():
             "schedule_used": {1: "thread", 2: "warp", 3: "cta"}[sched], "clocks": clocks, "e2e": e2e, "farm": farm,
             "kernel_ms_from": "separate timed steps (library events force a sync)" if tiny else "the timed steps",
             "adaptive": adaptive, "gpu_launches": launches,
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
-                         "frac": achieved / PEAK_GLANE, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+            # `frac` is the PHYSICAL-UNIT bound: algorithmic instruction counts x the pipe occupancy ncu measured per class, busiest
+            # unit (round 3; rounds 1-2 headlined the dispatch model, kept as frac_dispatch_model: ncu shows the FMA-heavy pipe
+            # only 82 % busy on a pure Philox block where that model claims the ceiling -- a fitted cost model, not a peak)
+            "roofline": {"bound": "alu", "achieved": pb_cyc * rate / 1e9, "peak": PEAK_GLANE, "unit": "G lane-cycles/s",
+                         "frac": pb_cyc * rate / 1e9 / PEAK_GLANE, "binding_unit": pb_bound, "unit_lane_cycles_per_eval": pb_res,
+                         "frac_dispatch_model": achieved / PEAK_GLANE, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
                          "traffic_source": NCU_TRAFFIC_SOURCE if w.name in NCU_TRAFFIC_BYTES else None,
                          # the same rate against SURVEY.md 8(d)'s own instruction table (see SURVEY_I_MIN above)
                          "frac_survey": sv_cyc * rate / 1e9 / PEAK_GLANE if sv else None,
@@ -439,12 +462,12 @@ def main():
                          "lane_cycles_per_eval": w_cyc, "binding_resource": w_bound, "resources": w_res,
                          "measured_lane_cycles_per_eval": PEAK_GLANE * 1e9 * (clocks["sm_mhz"] or SM_MAX_MHZ) / SM_MAX_MHZ / rate,
                          "lane_cycles_per_eval_no_overlap": w_add, "frac_no_overlap": w_add * rate / 1e9 / PEAK_GLANE,
-                         "peak_source": "peak = 148 SMs x 4 SMSPs x 32 lanes x 1965 MHz dispatch slots (sm_max_mhz of MEASURED_PEAKS.json; "
-                                        "its HBM / bf16 figures do not apply: ALU-bound, no contraction). `frac` counts the builder's W_min "
-                                        "(serial-dispatch model: integer 2, FP32 1 lane-cycles on one port; per-class costs re-measured in "
-                                        "this run, pipe_rates; DESIGN.md section 6). `frac_survey` counts SURVEY.md 8(d)'s table: "
-                                        "max(I_min, 4 x IMAD.WIDE) lane-cycles per evaluation",
-                         "frac_at_measured_clock": (achieved / (PEAK_GLANE * clocks["sm_mhz"] / SM_MAX_MHZ)
+                         "peak_source": "peak = 148 SMs x 4 SMSPs x 32 lanes x 1965 MHz (sm_max_mhz of MEASURED_PEAKS.json; its HBM / bf16 "
+                                        "figures do not apply: ALU-bound, no contraction). `frac`: algorithmic instruction list x per-class pipe "
+                                        "occupancy measured with ncu (profiles/r03_probe_ncu.md), busiest physical unit. `frac_dispatch_model`: "
+                                        "the builder's W_min (integer 2 + FP32 1 lane-cycles on one port; pipe_rates of this run; DESIGN.md "
+                                        "section 6). `frac_survey`: SURVEY.md 8(d)'s own table, max(I_min, 4 x IMAD.WIDE)",
+                         "frac_at_measured_clock": (pb_cyc * rate / 1e9 / (PEAK_GLANE * clocks["sm_mhz"] / SM_MAX_MHZ)
                                                     if clocks.get("sm_mhz") else None)},
         }
 
@@ -487,9 +510,10 @@ def main():
         "roofline": main_rec["roofline"],
     }
     if per_config:
-        out["per_config"] = {"columns": ["evals_per_s", "kernel_ms", "roofline_frac", "roofline_frac_survey", "e2e_evals_per_s"],
+        out["per_config"] = {"columns": ["evals_per_s", "kernel_ms", "roofline_frac", "frac_dispatch_model", "frac_survey", "e2e_evals_per_s"],
                              **{k: [float("%.4g" % v["value"]), round(v["kernel_ms_per_step"], 4), round(v["roofline"]["frac"], 3),
-                                    round(v["roofline"]["frac_survey"], 3), float("%.4g" % v["e2e"]["value"]) if v["e2e"] else None]
+                                    round(v["roofline"]["frac_dispatch_model"], 3), round(v["roofline"]["frac_survey"], 3),
+                                    float("%.4g" % v["e2e"]["value"]) if v["e2e"] else None]
                                 for k, v in per_config.items()}}
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(w)

@@ -46,6 +46,7 @@ thread_local int tl_cuda_error = 0;
 
 zmc_status cuda_fail(cudaError_t e) {
     tl_cuda_error = (int)e;
+    cudaGetLastError();      // the runtime remembers a failed call until asked: left there, the NEXT kernel launch's error check would report it
     return (e == cudaErrorMemoryAllocation) ? ZMC_ERR_OUT_OF_MEMORY : ZMC_ERR_CUDA;
 }
 }  // namespace
@@ -606,20 +607,36 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
     constexpr size_t kDirectBytes = 1u << 20;
     bool direct = false;
     uint64_t direct_bytes = 0;
+    uint32_t* direct_out_n = nullptr;
     if (host_out) {
-        cudaPointerAttributes pa, pb, pc;
+        // Device alias of a page-locked, mapped host range, or NULL.  Both ends of the range are looked up: a buffer that
+        // only STARTS in registered memory (a slice near the end of a cudaHostRegister'ed region, pageable memory behind
+        // it) must take the staged path -- the kernel would fault on the part that is not mapped.
+        auto mapped_alias = [](const void* host_ptr, size_t bytes) -> void* {
+            cudaPointerAttributes first, last;
+            if (bytes == 0 || cudaPointerGetAttributes(&first, host_ptr) != cudaSuccess || first.type != cudaMemoryTypeHost ||
+                !first.devicePointer) return nullptr;
+            if (cudaPointerGetAttributes(&last, static_cast<const char*>(host_ptr) + bytes - 1) != cudaSuccess ||
+                last.type != cudaMemoryTypeHost || !last.devicePointer) return nullptr;
+            if (static_cast<char*>(last.devicePointer) - static_cast<char*>(first.devicePointer) != (ptrdiff_t)(bytes - 1)) return nullptr;
+            return first.devicePointer;
+        };
+        cudaPointerAttributes pa;
         const bool pinned = cudaPointerGetAttributes(&pa, out_mean) == cudaSuccess && pa.type == cudaMemoryTypeHost;
         cudaGetLastError();
         if (timing) timing->host_out_pinned = pinned ? 1 : 0;   // copies into pageable memory run synchronously on the host
         direct_bytes = count * (elem_out * 2 + (ad ? sizeof(uint32_t) : 0));
-        if (pinned && n_batches == 1 && direct_bytes <= kDirectBytes && pa.devicePointer &&
-            cudaPointerGetAttributes(&pb, out_stderr) == cudaSuccess && pb.type == cudaMemoryTypeHost && pb.devicePointer &&
-            (!ad || (cudaPointerGetAttributes(&pc, ad->out_n) == cudaSuccess && pc.type == cudaMemoryTypeHost && pc.devicePointer))) {
-            direct = true;
-            host_out = false;                                   // from here on: an ordinary one-batch scan into "device" pointers
-            out_mean = pa.devicePointer;
-            out_stderr = pb.devicePointer;
-            if (timing) timing->host_out_pinned = 2;            // 2 = pinned and written directly by the kernel
+        if (pinned && n_batches == 1 && direct_bytes <= kDirectBytes) {
+            void* d_mean = mapped_alias(out_mean, (size_t)count * elem_out);
+            void* d_err = d_mean ? mapped_alias(out_stderr, (size_t)count * elem_out) : nullptr;
+            direct_out_n = (d_err && ad) ? static_cast<uint32_t*>(mapped_alias(ad->out_n, (size_t)count * sizeof(uint32_t))) : nullptr;
+            if (d_mean && d_err && (!ad || direct_out_n)) {
+                direct = true;
+                host_out = false;                                   // from here on: an ordinary one-batch scan into "device" pointers
+                out_mean = d_mean;
+                out_stderr = d_err;
+                if (timing) timing->host_out_pinned = 2;            // 2 = pinned and written directly by the kernel
+            }
         }
         cudaGetLastError();
     }
@@ -645,11 +662,7 @@ zmc_status scan_impl(int integrand_id, int N, const double* bounds, int M, const
                            : (schedule == ZMC_SCHED_WARP || schedule == kSchedAdapt) ? kThreads / 32 : 1;
     if (ad) {
         p.n_max = (uint32_t)ad->n_max; p.target = ad->target; p.out_n = ad->out_n;
-        if (direct) {                                           // the device alias of the caller's host array
-            cudaPointerAttributes pc;
-            ZMC_CUDA(cudaPointerGetAttributes(&pc, ad->out_n));
-            p.out_n = static_cast<uint32_t*>(pc.devicePointer);
-        }
+        if (direct) p.out_n = direct_out_n;                     // the device alias of the caller's host array
     }
     constexpr uint64_t kMaxLaunchPoints = 1ull << 30;
 

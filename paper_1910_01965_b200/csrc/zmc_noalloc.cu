@@ -73,6 +73,7 @@ std::mutex g_setup_mutex;
 
 zmc_status cuda_fail(cudaError_t e) {
     set_last_cuda_error((int)e);
+    cudaGetLastError();      // do not leave the failed call in the runtime's last-error slot for the next launch to find
     return ZMC_ERR_CUDA;
 }
 #define ZMC_CUDA(call)                                   \

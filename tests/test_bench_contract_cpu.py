@@ -38,6 +38,12 @@ def test_roofline_table_matches_design():
         cyc, b, res, no_overlap = bench.w_min(name)
         assert (cyc, b) == (w, bound) and no_overlap >= cyc
     assert abs(bench.PEAK_GLANE - 148 * 128 * 1.965) < 1e-6
+    # the physical-unit bound the line headlines (round-3 table; profiles/r03_probe_ncu.md)
+    want_pipes = {"cfg1": (30, "fp64"), "cfg2": (39, "issue"), "cfg3": (68, "fma_heavy"), "cfg4": (102.5, "fma_heavy"),
+                  "cfg5": (57, "fma_heavy"), "eq4": (96, "fma_heavy")}
+    for name, (cyc, unit) in want_pipes.items():
+        got, bound, res = bench.pipe_bound(name)
+        assert got == cyc and bound.startswith(unit) and got <= bench.w_min(name)[0]     # never looser than the dispatch model
     w = bench.build_workload("eq4_all", 1)
     assert w.G == 10 ** 8 and w.batch_points == 10 ** 6 and bench.config_of(w, 1)["scanned_points"] == 10 ** 8
     w8 = bench.build_workload("cfg5", 8)                                                # weak scaling: 8-fold first list

@@ -232,6 +232,48 @@ def test_small_one_batch_host_scans_are_written_by_the_kernel_itself():
     assert torch.equal(n_h, n_d.cpu()) and torch.equal(hm[32:32 + w.G], am.cpu()) and torch.equal(he[32:32 + w.G], ae.cpu())
 
 
+def test_host_buffers_that_only_start_in_page_locked_memory_do_not_take_the_direct_path():
+    """A result buffer whose first bytes lie in a cudaHostRegister'ed region but whose end runs past it (a slice near the end
+    of a registered range, pageable memory behind it) must not be written by the kernel through the mapped alias: the part
+    that is not mapped would fault the kernel and poison the context.  It goes through the staged copies instead; whatever
+    the runtime makes of a copy into such a range (it may also refuse it), the library stays usable."""
+    import mmap
+    import torch
+    from paper_1910_01965_b200 import binding as zb
+    w = wl.config(2, scale=[37, 29], n_samples=300)                       # 1073 points x 8 B per array
+    dm, de, _ = zb.scan_workload(w, host_out=False)
+    page = mmap.PAGESIZE
+    bufs, arrays = [], []
+    rt = torch.cuda.cudart()
+    for _ in range(2):
+        mm = mmap.mmap(-1, 8 * page)
+        arr = np.frombuffer(mm, dtype=np.float64)
+        arr[:] = -7.0
+        assert int(rt.cudaHostRegister(arr.ctypes.data, 2 * page, 1)) == 0          # only the first two pages are page-locked
+        bufs.append(mm)
+        arrays.append(arr)
+    start = (2 * page - 1024) // 8                                         # the last KiB of the registered part ...
+    hm, he = (torch.from_numpy(a)[start:start + w.G] for a in arrays)      # ... and 7.5 KiB of pageable memory behind it
+    try:
+        import warnings
+        with warnings.catch_warnings():
+            warnings.simplefilter("ignore")
+            try:
+                _, _, tm = zb.scan_workload(w, out_mean=hm, out_stderr=he, host_out=True, batch_points=0, timing=True)
+                torch.cuda.synchronize()
+                assert tm["host_out_pinned"] != 2                          # not the direct path
+                assert torch.equal(hm, dm.cpu()) and torch.equal(he, de.cpu())
+            except zb.ZmcError as exc:                                     # a clean refusal of the copy is acceptable too
+                assert exc.status == zb.ZMC_ERR_CUDA
+        torch.cuda.synchronize()                                           # no sticky error: the context still works
+        dm2, de2, _ = zb.scan_workload(w, host_out=False)
+        torch.cuda.synchronize()
+        assert torch.equal(dm2, dm) and torch.equal(de2, de)
+    finally:
+        for a in arrays:
+            rt.cudaHostUnregister(a.ctypes.data)
+
+
 def test_a_scan_with_device_outputs_can_be_captured_into_a_cuda_graph():
     """A scan into device memory whose value lists are already cached on the device enqueues one kernel and one event record
     on the caller's stream (include/zmc.h, zmc_scan_ex): it can be captured into a CUDA graph and replayed, and ordinary
